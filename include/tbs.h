@@ -1,0 +1,141 @@
+/*
+ * tbs.h -- C ABI of libtbs: traditional Born series (TBS) solve of the inhomogeneous Helmholtz
+ * equation on one B200 (sm_100a).  Paper: arxiv 2507.13754 (citations: PAPER.md line numbers).
+ *
+ *   psi = G V psi + G S                      (Eq. 17)
+ *   psi = [1 + GV + GVGV + ...] G S          (Eq. 18)  -- summed term by term:
+ *   u_0 = A.(G S), u_{n+1} = A.G(V.u_n), p = sum_n u_n
+ *   G = crop . IDFT_2N . ghat(p) . DFT_2N . zero-pad,  ghat = 1/(|p|^2 - k0^2 - i eps)
+ *   V(r) = ktilde(r)^2 - k0^2 - i eps, eps = damping k0^2
+ *
+ * Conventions
+ *  - Every array is row-major with x fastest: index = (z*Ny + y)*Nx + x.
+ *  - complex64 = interleaved float (re, im).  "dev" = CUDA device pointer, "host" = host pointer.
+ *  - The caller owns every buffer it passes in.  The plan owns V, S, p and the FFT workspaces.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - No exception crosses the ABI: every call returns a tbs_status; tbs_last_error() gives text.
+ *  - A plan is not thread-safe; distinct plans are independent.
+ *  - Grid sizes: every n[i] a power of two, 32 <= n[i] <= 4096 (2-D), 32 <= n[i] <= 512 (3-D),
+ *    else TBS_ERR_UNSUPPORTED_SIZE.  The padded length is 2 n[i] per axis and is never
+ *    materialised in more than one axis beyond what a pass needs.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns TBS_ERR_CUDA.
+ */
+#ifndef TBS_H_
+#define TBS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tbs_plan tbs_plan;
+
+typedef enum {
+    TBS_OK = 0,
+    TBS_NOT_CONVERGED = 1,       /* max_terms reached: field and history are valid */
+    TBS_ERR_INVALID_ARG = -1,
+    TBS_ERR_UNSUPPORTED_SIZE = -2,
+    TBS_ERR_NOT_READY = -3,      /* medium or source not set */
+    TBS_ERR_CUDA = -4,
+    TBS_ERR_DIVERGED = -5,       /* a term norm became non-finite (||GV|| >= 1) */
+    TBS_ERR_ALLOC = -6
+} tbs_status;
+
+/* Library version string (static storage). */
+const char *tbs_version(void);
+
+/* Create a plan for one grid and nfreq frequencies (Alg. 1 Input).
+ *   ndim: 2 or 3.  n: grid points per axis in x, y, z order (n[2] ignored for ndim = 2).
+ *   dx_m: grid spacing (m), equal on all axes.  f_hz[nfreq]: frequencies (host).
+ *   c0: reference sound speed (m/s), k0 = 2 pi f/c0.
+ *   damping: eps/k0^2, the paper uses 0.8.
+ * Builds the per-axis |p|^2 tables and twiddles (Green's-spectrum precompute)
+ * and allocates device workspaces.  *out is NULL on failure. */
+tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double dx_m, int nfreq,
+                           const double *f_hz, double c0, double damping);
+void tbs_plan_destroy(tbs_plan *plan);
+
+/* Device bytes the plan holds (fields + workspaces). */
+size_t tbs_plan_workspace_bytes(const tbs_plan *plan);
+
+/* Text of the last error on this plan (plan-owned storage, valid until the next call). */
+const char *tbs_last_error(const tbs_plan *plan);
+
+/* Absorbing layer of Eq. 29 on all faces, `cells` wide, window
+ * 1/(1+exp(-zeta (x - mu/2))) with zeta*mu/2 = zeta_half_mu (paper: 9.666).  cells = 0 (default)
+ * is the pure zero-pad/crop boundary.  Folded into the crop kernel as per-axis factors. */
+tbs_status tbs_set_abl(tbs_plan *plan, int cells, double zeta_half_mu);
+
+/* Medium -> potential, for every frequency of the plan (absorption from
+ * Eq. 3 and Eq. 7):
+ *   ktilde = w/c(r) + alpha (tan(pi y/2) + i), alpha = alpha0 w^y, V = ktilde^2 - k0^2 - i eps.
+ *   c [n] dev float: sound speed map.  rho [n] dev float or NULL: density; it does not enter V
+ *   (rho_s ~ rho_f); its mean (or rho0 when NULL) enters the harmonic source only.
+ *   alpha0_map [n] dev float or NULL (then the scalar alpha0_db_mhz_cm is used), dB/(MHz^y cm).
+ *   y: power-law exponent, y != 1 unless alpha0 == 0.  beta = 1 + B/2A.
+ * tbs_set_medium_host takes the same maps as HOST pointers and copies them itself. */
+tbs_status tbs_set_medium(tbs_plan *plan, const float *c, const float *rho, const float *alpha0_map,
+                          double alpha0_db_mhz_cm, double y, double beta, double rho0, void *stream);
+tbs_status tbs_set_medium_host(tbs_plan *plan, const float *c, const float *rho,
+                               const float *alpha0_map, double alpha0_db_mhz_cm, double y,
+                               double beta, double rho0, void *stream);
+
+/* Raw potential for frequency ifreq (test hook and user-supplied V): V [n][2] dev, in 1/m^2,
+ * must already include the -i eps term. */
+tbs_status tbs_set_potential(tbs_plan *plan, int ifreq, const float *V, void *stream);
+
+/* Point sources (transducer elements): pos_m [n_src][ndim] host doubles in
+ * (x, y[, z]) order, centre of cell (0,0,0) at r = 0; amp [nfreq][n_src][2] host floats (re, im).
+ * Off-grid points are deposited with multilinear weights; a point on a node is the paper's
+ * single-pixel source.  A point outside the grid gives TBS_ERR_INVALID_ARG. */
+tbs_status tbs_set_source(tbs_plan *plan, int n_src, const double *pos_m, const float *amp,
+                          void *stream);
+/* Dense source density for frequency ifreq: S [n][2] dev. */
+tbs_status tbs_set_source_field(tbs_plan *plan, int ifreq, const float *S, void *stream);
+
+/* Run the series for every frequency until history < tol, max_terms, or divergence.
+ *   p_out [nfreq][n][2]: dev (tbs_solve) or host (tbs_solve_host) complex64 field.
+ *   history [nfreq][max_terms+1] host doubles: history[k] = ||u_k||_2/||p_k||_2, history[0] = 1;
+ *     entries after n_terms are 0.   n_terms [nfreq] host: index of the last term added.
+ * Synchronises `stream` before returning.  Returns the worst status over frequencies. */
+tbs_status tbs_solve(tbs_plan *plan, int max_terms, double tol, float *p_out, double *history,
+                     int32_t *n_terms, void *stream);
+tbs_status tbs_solve_host(tbs_plan *plan, int max_terms, double tol, float *p_out_host,
+                          double *history, int32_t *n_terms, void *stream);
+
+/* Nonlinear case (Eq. 27b, 229 Eq. 28b, 266): solve `p1` (fundamental, nfreq = 1),
+ * optionally rescale it so that max|p1| over the row/plane `ref_row` equals surface_pressure_pa
+ * (<= 0: no rescale), form S2 = -xi (2w)^2 p1^2/2 with xi = beta/(rho0 c0^4), and solve `p2`
+ * (a plan created at 2 f on the same grid, medium already set).  Outputs as tbs_solve, once for
+ * each plan; p1_out / p2_out [n][2] dev. */
+tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, double tol,
+                                     int ref_row, double surface_pressure_pa, float *p1_out,
+                                     float *p2_out, double *history1, double *history2,
+                                     int32_t *n_terms1, int32_t *n_terms2, void *stream);
+
+/* Introspection for tests and the bench. */
+/* One application of G to x (dev [n][2]) for frequency ifreq: out = crop IDFT ghat DFT pad x. */
+tbs_status tbs_apply_green(tbs_plan *plan, int ifreq, const float *x, float *out, void *stream);
+/* Copy the plan's V or S for frequency ifreq to dev buffer out [n][2]. */
+tbs_status tbs_get_potential(tbs_plan *plan, int ifreq, float *out, void *stream);
+tbs_status tbs_get_source(tbs_plan *plan, int ifreq, float *out, void *stream);
+/* Full Green's spectrum ghat on the padded grid in natural FFT order, dev [prod(2 n[i])][2]
+ * (the tabulated form of the precompute kernel; the hot path recomputes ghat from axis tables). */
+tbs_status tbs_green_spectrum(tbs_plan *plan, int ifreq, float *out, void *stream);
+/* Kernel launches issued by the last tbs_solve* on this plan, and device time (ms) of its term
+ * loop measured with CUDA events on `stream`. */
+int64_t tbs_last_launch_count(const tbs_plan *plan);
+double tbs_last_loop_ms(const tbs_plan *plan);
+/* Per-kernel device time of ONE term (ms) for frequency ifreq, measured with CUDA events around
+ * `reps` back-to-back launches of each kernel: out_ms[0..3] = row kernel K31, column/plane
+ * passes K2 (2-D) or Ky-fwd, Kz, Ky-inv (3-D: out_ms[1..3]).  Requires medium and source. */
+tbs_status tbs_profile_term(tbs_plan *plan, int ifreq, int reps, double out_ms[4], void *stream);
+/* Terms per graph launch (default 16); 0 disables CUDA graphs (plain launches). */
+tbs_status tbs_set_graph_batch(tbs_plan *plan, int terms_per_graph);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TBS_H_ */

@@ -1,0 +1,217 @@
+// fft_engine.cuh -- in-place shared-memory FFT building blocks for the TBS kernels (sm_100a).
+//
+// A length-N complex FFT (N = 2^n, 32..4096) is factored as N = R1 * [R2] * RL with radices in
+// {4, 8, 16}.  Forward transforms are decimation-in-frequency (natural order in, digit-reversed
+// order out), inverse transforms are the mirrored decimation-in-time (digit-reversed in, natural
+// out), so no reorder pass ever runs: the Green's spectrum ghat(p) is even in every
+// component of p and is simply indexed in the scrambled order (tables are built in "position
+// order" on the host).  Data lives in shared memory between stages; every stage reads and writes
+// the same positions ("in place"), so one __syncthreads() separates two stages.
+//
+// Zero padding N -> M = 2N (BASELINE.json north_star) is never materialised:
+//   X[2k+s] = sum_{j<N} (x[j] w_M^{js}) w_N^{jk}            (forward, s = 0, 1: two length-N FFTs)
+//   y[j]    = sum_s w_M^{-js} IFFT_N(Y[2k+s])[j],  j < N     (inverse followed by the crop)
+// so a padded line is stored as two halves of N "positions": P = s*N + pos.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tbs {
+
+constexpr int NTW = 8192;  // twiddle table length: tw[k] = exp(-2 pi i k / NTW)
+
+// ---- complex helpers -------------------------------------------------------------------------
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// a * conj(b)
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) {
+    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+
+// ---- radix plan ------------------------------------------------------------------------------
+template <int N> struct Radix;
+template <> struct Radix<32>   { static constexpr int R1 = 8,  R2 = 0,  RL = 4;  };
+template <> struct Radix<64>   { static constexpr int R1 = 8,  R2 = 0,  RL = 8;  };
+template <> struct Radix<128>  { static constexpr int R1 = 16, R2 = 0,  RL = 8;  };
+template <> struct Radix<256>  { static constexpr int R1 = 16, R2 = 0,  RL = 16; };
+template <> struct Radix<512>  { static constexpr int R1 = 8,  R2 = 8,  RL = 8;  };
+template <> struct Radix<1024> { static constexpr int R1 = 16, R2 = 8,  RL = 8;  };
+template <> struct Radix<2048> { static constexpr int R1 = 16, R2 = 16, RL = 8;  };
+template <> struct Radix<4096> { static constexpr int R1 = 16, R2 = 16, RL = 16; };
+
+__host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
+// bit reversal of i within log2(R) bits
+__host__ __device__ constexpr int brev(int i, int R) {
+    int r = 0;
+    for (int b = 1; b < R; b <<= 1) { r = (r << 1) | (i & 1); i >>= 1; }
+    return r;
+}
+
+// ---- radix-R butterfly in registers ----------------------------------------------------------
+// d * w_16^(idx16) with sign SGN (SGN = -1: exp(-2 pi i idx/16), forward; +1: inverse).
+template <int SGN>
+__device__ __forceinline__ float2 mul_w16(float2 d, int idx16) {
+    constexpr float C1 = 0.92387953251128674f;  // cos(pi/8)
+    constexpr float S1 = 0.38268343236508977f;  // sin(pi/8)
+    constexpr float H = 0.70710678118654752f;   // sqrt(1/2)
+    const float s = (float)SGN;
+    switch (idx16) {
+        case 0: return d;
+        case 1: return make_float2(d.x * C1 - s * d.y * S1, d.y * C1 + s * d.x * S1);
+        case 2: return make_float2((d.x - s * d.y) * H, (d.y + s * d.x) * H);
+        case 3: return make_float2(d.x * S1 - s * d.y * C1, d.y * S1 + s * d.x * C1);
+        case 4: return make_float2(-s * d.y, s * d.x);
+        case 5: return make_float2(-d.x * S1 - s * d.y * C1, -d.y * S1 + s * d.x * C1);
+        case 6: return make_float2((-d.x - s * d.y) * H, (-d.y + s * d.x) * H);
+        default: return make_float2(-d.x * C1 - s * d.y * S1, -d.y * C1 + s * d.x * S1);
+    }
+}
+
+// DFT_R of v (sign SGN), natural order in, BIT-REVERSED order out: v[i] <- X[brev(i, R)].
+template <int R, int SGN>
+__device__ __forceinline__ void bfly(float2 (&v)[R]) {
+#pragma unroll
+    for (int h = R / 2; h >= 1; h >>= 1) {
+#pragma unroll
+        for (int g = 0; g < R; g += 2 * h) {
+#pragma unroll
+            for (int m = 0; m < h; ++m) {
+                float2 a = v[g + m], b = v[g + m + h];
+                v[g + m] = cadd(a, b);
+                v[g + m + h] = mul_w16<SGN>(csub(a, b), m * (8 / h));
+            }
+        }
+    }
+}
+
+// ---- shared-memory layouts -------------------------------------------------------------------
+// Column tile: T adjacent lines interleaved, [pos][T].  A warp covers 32/T positions x T lines.
+// XOR swizzle of the low position bits keeps the contiguous-block stage (stride RL between
+// lanes) conflict-free for T < 16.
+template <int N, int T_, int RL>
+struct ColLay {
+    static constexpr int T = T_;
+    static constexpr int G = (16 / T_ > 1) ? 16 / T_ : 1;
+    static constexpr int SMEM_ELEMS = N * T_;
+    __device__ static __forceinline__ int addr(int line, int pos) {
+        if (G > 1) pos ^= (pos / RL) & (G - 1);
+        return pos * T_ + line;
+    }
+    template <int NBL>
+    __device__ static __forceinline__ void split(int w, int &line, int &b) { line = w % T_; b = w / T_; }
+};
+// Row tile: each line contiguous, one pad slot per 16 positions.
+template <int N>
+struct RowLay {
+    static constexpr int PITCH = N + N / 16;
+    __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + pos + (pos >> 4); }
+    template <int NBL>
+    __device__ static __forceinline__ void split(int w, int &line, int &b) { b = w % NBL; line = w / NBL; }
+};
+
+// ---- generic in-place stage on shared memory ---------------------------------------------------
+// Block length LB, radix R, sub-stride S = LB/R.  DIF: butterfly then twiddle w_LB^(k t);
+// DIT (inverse): conj twiddle then butterfly.  `total` = number of butterflies in the tile.
+template <int N, int LB, int R, bool FWD, class Lay, int NT>
+__device__ __forceinline__ void stage_smem(float2 *sm, const float2 *__restrict__ tw, int tid, int total) {
+    constexpr int S = LB / R;
+    constexpr int NBL = N / R;
+    for (int w = tid; w < total; w += NT) {
+        int line, b;
+        Lay::template split<NBL>(w, line, b);
+        const int t = b % S;
+        const int base = (b / S) * LB + t;
+        float2 v[R];
+        if (FWD) {
+#pragma unroll
+            for (int j = 0; j < R; ++j) v[j] = sm[Lay::addr(line, base + j * S)];
+            bfly<R, -1>(v);
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const int k = brev(i, R);
+                float2 o = v[i];
+                if (S > 1 && k > 0) o = cmul(o, __ldg(&tw[k * t * (NTW / LB)]));
+                sm[Lay::addr(line, base + k * S)] = o;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < R; ++k) {
+                float2 x = sm[Lay::addr(line, base + k * S)];
+                if (S > 1 && k > 0) x = cmulc(x, __ldg(&tw[k * t * (NTW / LB)]));
+                v[k] = x;
+            }
+            bfly<R, +1>(v);
+#pragma unroll
+            for (int i = 0; i < R; ++i) sm[Lay::addr(line, base + brev(i, R) * S)] = v[i];
+        }
+    }
+}
+
+// First forward stage from registers: x[j] sits at position t + j*S1 (natural order).
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void first_fwd(float2 (&x)[R1], int line, int t, float2 *sm,
+                                          const float2 *__restrict__ tw) {
+    constexpr int S1 = N / R1;
+    bfly<R1, -1>(x);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) {
+        const int k = brev(i, R1);
+        float2 o = x[i];
+        if (k > 0) o = cmul(o, __ldg(&tw[k * t * (NTW / N)]));
+        sm[Lay::addr(line, t + k * S1)] = o;
+    }
+}
+
+// Last inverse stage into registers: z[j] is the (unnormalised) inverse at position t + j*S1.
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void last_inv(float2 (&z)[R1], int line, int t, const float2 *sm,
+                                         const float2 *__restrict__ tw) {
+    constexpr int S1 = N / R1;
+    float2 v[R1];
+#pragma unroll
+    for (int k = 0; k < R1; ++k) {
+        float2 x = sm[Lay::addr(line, t + k * S1)];
+        if (k > 0) x = cmulc(x, __ldg(&tw[k * t * (NTW / N)]));
+        v[k] = x;
+    }
+    bfly<R1, +1>(v);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) z[brev(i, R1)] = v[i];
+}
+
+// Fused middle of the convolution: last forward stage (contiguous blocks of RL), multiply by
+// ghat, first inverse stage -- all in registers (north_star: "pointwise G multiply fused into the
+// last forward and first inverse butterfly stage").
+//   ghat' = scale / (a - i e),  a = a_line + p2[P],  e = eps/k0^2   (non-dimensional)
+template <int N, int RL, class Lay, int NT>
+__device__ __forceinline__ void mid_conv(float2 *sm, int tid, int total, const float *__restrict__ p2half,
+                                         float a_line, float e, float scale) {
+    constexpr int NBL = N / RL;
+    const float e2 = e * e;
+    for (int w = tid; w < total; w += NT) {
+        int line, b;
+        Lay::template split<NBL>(w, line, b);
+        const int base = b * RL;
+        float2 v[RL];
+#pragma unroll
+        for (int j = 0; j < RL; ++j) v[j] = sm[Lay::addr(line, base + j)];
+        bfly<RL, -1>(v);
+        float2 u[RL];
+#pragma unroll
+        for (int i = 0; i < RL; ++i) {
+            const int k = brev(i, RL);
+            const float a = a_line + __ldg(&p2half[base + k]);
+            const float r = __fdiv_rn(scale, fmaf(a, a, e2));
+            const float gr = a * r, gi = e * r;
+            u[k] = make_float2(v[i].x * gr - v[i].y * gi, v[i].x * gi + v[i].y * gr);
+        }
+        bfly<RL, +1>(u);
+#pragma unroll
+        for (int i = 0; i < RL; ++i) sm[Lay::addr(line, base + brev(i, RL))] = u[i];
+    }
+}
+
+}  // namespace tbs

@@ -1,0 +1,151 @@
+// setup_kernels.cuh -- once-per-plan / once-per-medium kernels.
+// All evaluate in double and store float, so the hot path sees correctly rounded inputs.
+#pragma once
+#include "fft_engine.cuh"
+
+namespace tbs {
+
+// tw[k] = exp(-2 pi i k / NTW)
+__global__ void k_twiddles(float2 *tw) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= NTW) return;
+    double s, c;
+    sincospi(-2.0 * (double)k / (double)NTW, &s, &c);
+    tw[k] = make_float2((float)c, (float)s);
+}
+
+// Frequency index held at `pos` of a length-N DIF transform with radices r1, r2 (0 = none), rl.
+__host__ __device__ inline int freq_of_pos(int pos, int N, int r1, int r2, int rl) {
+    const int s1 = N / r1;
+    const int k1 = pos / s1;
+    int rem = pos % s1;
+    if (r2 > 0) {
+        const int s2 = s1 / r2;
+        const int k2 = rem / s2;
+        const int k3 = rem % s2;
+        return k1 + r1 * (k2 + r2 * k3);
+    }
+    return k1 + r1 * rem;
+}
+
+// Green's-spectrum axis table (Alg. 1 l.9-10, in FFT order rather than centred +
+// fftShift): p2[P] = (2 pi F~/(M dx))^2 / k0^2 with P = s*N + pos the position that
+// holds padded-grid frequency F = 2 freqN(pos) + s, F~ = F for F < M/2, F - M otherwise.
+__global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0) {
+    const int P = blockIdx.x * blockDim.x + threadIdx.x;
+    const int M = 2 * N;
+    if (P >= M) return;
+    const int s = P / N, pos = P % N;
+    const int F = 2 * freq_of_pos(pos, N, r1, r2, rl) + s;
+    const double Ft = (F < M / 2) ? (double)F : (double)(F - M);
+    const double p = 2.0 * 3.14159265358979323846 * Ft / ((double)M * dx);
+    p2[P] = (float)((p * p) / (k0 * k0));
+}
+
+// Full Green's spectrum in natural FFT order, ghat = ((p2-k0^2) + i eps)/((p2-k0^2)^2 + eps^2)
+// exactly as Alg. 1 l.12.  Tabulated form for inspection; the hot path recomputes
+// ghat from the axis tables.
+__global__ void k_green_spectrum(float2 *g, int mx, int my, int mz, double dx, double k0, double eps) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long tot = (long long)mx * my * mz;
+    if (i >= tot) return;
+    const int ix = (int)(i % mx), iy = (int)((i / mx) % my), iz = (int)(i / ((long long)mx * my));
+    const double tp = 2.0 * 3.14159265358979323846;
+    const double px = tp * (double)(ix < mx / 2 ? ix : ix - mx) / ((double)mx * dx);
+    const double py = my > 1 ? tp * (double)(iy < my / 2 ? iy : iy - my) / ((double)my * dx) : 0.0;
+    const double pz = mz > 1 ? tp * (double)(iz < mz / 2 ? iz : iz - mz) / ((double)mz * dx) : 0.0;
+    const double a = px * px + py * py + pz * pz - k0 * k0;
+    const double D = a * a + eps * eps;
+    g[i] = make_float2((float)(a / D), (float)(eps / D));
+}
+
+// Medium -> non-dimensional potential V/k0^2 (absorption reading A6):
+//   ktilde = w/c + alpha (tan(pi y/2) + i), alpha = alpha0_SI w^y, V = ktilde^2 - k0^2 - i eps.
+__global__ void k_potential(float2 *V, const float *c, const float *alpha0_map, double alpha0_db,
+                            double y, double omega, double k0, double damping, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double a0 = alpha0_map ? (double)alpha0_map[i] : alpha0_db;
+    double kr = omega / (double)c[i], ki = 0.0;
+    if (a0 != 0.0) {
+        const double a0si = a0 * 100.0 / 8.685889638 / pow(2.0 * 3.14159265358979323846 * 1.0e6, y);
+        const double alpha = a0si * pow(omega, y);
+        kr += alpha * tan(3.14159265358979323846 * y / 2.0);
+        ki = alpha;
+    }
+    const double k2 = k0 * k0;
+    V[i] = make_float2((float)((kr * kr - ki * ki - k2) / k2), (float)((2.0 * kr * ki) / k2 - damping));
+}
+
+// Raw V (1/m^2) -> V/k0^2
+__global__ void k_scale_complex(float2 *dst, const float2 *src, double s, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    dst[i] = make_float2((float)((double)src[i].x * s), (float)((double)src[i].y * s));
+}
+
+// Source deposition with multilinear weights (reading A9; a node-aligned point is the paper's
+// single-pixel source).  One thread per (source, corner).
+__global__ void k_deposit(float2 *S, const double *pos, const float2 *amp, int n_src, int ndim,
+                          int nx, int ny, int nz, double dx) {
+    const int corners = 1 << ndim;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_src * corners) return;
+    const int j = i / corners, cidx = i % corners;
+    const int dims[3] = {nx, ny, nz};
+    long long idx = 0, stride = 1;
+    double w = 1.0;
+    for (int a = 0; a < ndim; ++a) {
+        const double g = pos[(long long)j * ndim + a] / dx;
+        double fl = floor(g);
+        if (fl > (double)(dims[a] - 2)) fl = (double)(dims[a] - 2);
+        const double fr = g - fl;
+        const int bit = (cidx >> a) & 1;
+        w *= bit ? fr : 1.0 - fr;
+        idx += ((long long)fl + bit) * stride;
+        stride *= dims[a];
+    }
+    if (w == 0.0) return;
+    atomicAdd(&S[idx].x, (float)((double)amp[j].x * w));
+    atomicAdd(&S[idx].y, (float)((double)amp[j].y * w));
+}
+
+// Absorbing-layer window along one axis, Eq. 29, reading A4.
+__global__ void k_abl_window(float *a, int n, int cells, double zeta_half_mu) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int x = i < n - 1 - i ? i : n - 1 - i;
+    double v = 1.0;
+    if (cells > 0 && x < cells) {
+        const double zeta = 2.0 * zeta_half_mu / (double)cells;
+        v = 1.0 / (1.0 + exp(-zeta * ((double)x - 0.5 * (double)cells)));
+    }
+    a[i] = (float)v;
+}
+
+// max |p|^2 over one row (2-D) / plane (3-D), as the bit pattern of a non-negative float.
+__global__ void k_row_max(const float2 *p, long long first, long long count, unsigned int *out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    float m = 0.f;
+    if (i < count) {
+        const float2 v = p[first + i];
+        m = v.x * v.x + v.y * v.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));
+}
+
+// p1 <- g p1 (g = target / max|p1| when target > 0), S2 = -xi (2 w1)^2 (1/2) p1^2
+// (Eq. 28b; xi = beta/(rho0 c0^4)).
+__global__ void k_second_harmonic_source(float2 *p1, float2 *S2, const unsigned int *max2bits,
+                                         double target, double coef, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double g = 1.0;
+    if (target > 0.0) g = target / sqrt((double)__uint_as_float(*max2bits));
+    const double re = (double)p1[i].x * g, im = (double)p1[i].y * g;
+    p1[i] = make_float2((float)re, (float)im);
+    S2[i] = make_float2((float)(coef * (re * re - im * im)), (float)(coef * 2.0 * re * im));
+}
+
+}  // namespace tbs

@@ -1,0 +1,226 @@
+// solve.inl -- the Born-term loop and its drivers (included at the end of tbs.cu).
+
+namespace {
+
+// Build (once) a CUDA graph holding `batch` terms for frequency f.
+tbs_status build_graph(tbs_plan *pl, Freq &f, int batch, cudaStream_t st) {
+    if (f.graph && f.graph_batch == batch) return TBS_OK;
+    if (f.graph) { cudaGraphExecDestroy(f.graph); f.graph = nullptr; }
+    cudaStream_t cs;
+    CU(pl, cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        for (int i = 0; i < batch && e == cudaSuccess; ++i) e = launch_term(pl, f, cs);
+        cudaError_t e2 = cudaStreamEndCapture(cs, &g);
+        if (e == cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&f.graph, g, 0);
+    if (g) cudaGraphDestroy(g);
+    cudaStreamDestroy(cs);
+    (void)st;
+    if (e != cudaSuccess) { f.graph = nullptr; return fail(pl, TBS_ERR_CUDA, "graph build: %s", cudaGetErrorString(e)); }
+    f.graph_batch = batch;
+    return TBS_OK;
+}
+
+// Run the series for one frequency.  The field is left in f.p, history in pl->h_hist.
+tbs_status solve_one(tbs_plan *pl, int ifreq, int max_terms, double tol, cudaStream_t st, int *n_terms_out) {
+    Freq &f = pl->fr[ifreq];
+    if (!f.have_V) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_medium / tbs_set_potential not called");
+    if (!f.have_S) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_source / tbs_set_source_field not called");
+    tbs_status hs = ensure_history(pl, max_terms);
+    if (hs != TBS_OK) return hs;
+    const int batch = pl->graph_batch > 0 ? pl->graph_batch : 8;
+    if (pl->graph_batch > 0) {
+        tbs_status gs = build_graph(pl, f, batch, st);
+        if (gs != TBS_OK) return gs;
+    }
+    Ctl *h = pl->h_ctl;
+    memset(&h[0], 0, sizeof(Ctl));
+    h[0].max_terms = max_terms;
+    h[0].tol = tol;
+    h[0].status = 1;
+    CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
+    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * (max_terms + 1), st));
+    CU(pl, cudaMemsetAsync(pl->history, 0, sizeof(double) * (max_terms + 1), st));
+    CU(pl, cudaEventRecord(pl->ev_t0, st));
+    // term 0 forward half: W = FFT_x(pad(S / k0^2))
+    RowArgs r;
+    fill_row_args(pl, f, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row<true>(pl->n[0], r, st));
+    pl->launches += 1;
+    const int per_term = mid_launches(pl) + 1;
+    // batches, double-buffered: enqueue batch i+1 before looking at the flag of batch i
+    int issued = 0;
+    bool done = false;
+    const int max_batches = (max_terms + 1 + batch - 1) / batch + 1;
+    for (int b = 0; b < max_batches + 1 && !done; ++b) {
+        if (b < max_batches) {
+            if (pl->graph_batch > 0) {
+                CU(pl, cudaGraphLaunch(f.graph, st));
+            } else {
+                for (int i = 0; i < batch; ++i) CU(pl, launch_term(pl, f, st));
+            }
+            pl->launches += (long long)batch * per_term;
+            CU(pl, cudaMemcpyAsync(&h[1 + (b & 1)], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+            CU(pl, cudaEventRecord(pl->ev[b & 1], st));
+            ++issued;
+        }
+        if (b >= 1) {
+            CU(pl, cudaEventSynchronize(pl->ev[(b - 1) & 1]));
+            if (h[1 + ((b - 1) & 1)].done) done = true;
+        }
+    }
+    CU(pl, cudaEventRecord(pl->ev_t1, st));
+    CU(pl, cudaMemcpyAsync(&h[3], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+    CU(pl, cudaMemcpyAsync(pl->h_hist, pl->history, sizeof(double) * (max_terms + 1), cudaMemcpyDeviceToHost, st));
+    CU(pl, cudaStreamSynchronize(st));
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, pl->ev_t0, pl->ev_t1);
+    pl->loop_ms += ms;
+    if (!h[3].done) return fail(pl, TBS_ERR_CUDA, "term loop ended without the stop flag (issued %d batches)", issued);
+    *n_terms_out = h[3].n_terms;
+    if (h[3].status == TBS_ERR_DIVERGED) fail(pl, TBS_ERR_DIVERGED, "term norm became non-finite at term %d", h[3].n_terms);
+    return (tbs_status)h[3].status;
+}
+
+tbs_status worst(tbs_status a, tbs_status b) {
+    if (a < 0) return a;
+    if (b < 0) return b;
+    return a > b ? a : b;
+}
+
+tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool out_is_host,
+                     double *history, int32_t *n_terms, cudaStream_t st) {
+    if (!pl || max_terms < 0 || !(tol >= 0) || !p_out || !history || !n_terms) return TBS_ERR_INVALID_ARG;
+    pl->launches = 0;
+    pl->loop_ms = 0;
+    tbs_status res = TBS_OK;
+    for (int i = 0; i < (int)pl->fr.size(); ++i) {
+        int nt = 0;
+        tbs_status s = solve_one(pl, i, max_terms, tol, st, &nt);
+        if (s < 0 && s != TBS_ERR_DIVERGED) return s;
+        n_terms[i] = nt;
+        double *hrow = history + (size_t)i * (max_terms + 1);
+        for (int k = 0; k <= max_terms; ++k) hrow[k] = k <= nt ? pl->h_hist[k] : 0.0;
+        CU(pl, cudaMemcpyAsync((float2 *)p_out + (size_t)i * pl->npts, pl->fr[i].p, sizeof(float2) * pl->npts,
+                               out_is_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+        res = worst(res, s);
+    }
+    CU(pl, cudaStreamSynchronize(st));
+    return res;
+}
+
+}  // namespace
+
+extern "C" {
+
+tbs_status tbs_solve(tbs_plan *pl, int max_terms, double tol, float *p_out, double *history,
+                     int32_t *n_terms, void *stream) {
+    return solve_all(pl, max_terms, tol, p_out, false, history, n_terms, (cudaStream_t)stream);
+}
+
+tbs_status tbs_solve_host(tbs_plan *pl, int max_terms, double tol, float *p_out_host, double *history,
+                          int32_t *n_terms, void *stream) {
+    return solve_all(pl, max_terms, tol, p_out_host, true, history, n_terms, (cudaStream_t)stream);
+}
+
+tbs_status tbs_apply_green(tbs_plan *pl, int ifreq, const float *x, float *out, void *stream) {
+    if (!pl || !x || !out || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    Freq &f = pl->fr[ifreq];
+    tbs_status hs = ensure_history(pl, 1);
+    if (hs != TBS_OK) return hs;
+    // Save the plan's running field: the inverse half writes p.
+    Ctl *h = pl->h_ctl;
+    memset(&h[0], 0, sizeof(Ctl));
+    h[0].max_terms = 1 << 30;
+    h[0].tol = 0.0;
+    CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
+    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
+    // Use `out` itself as the field buffer and a unit window-free pass: A is applied (as in u_0).
+    RowArgs r;
+    fill_row_args(pl, f, r, (const float2 *)x, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row<true>(pl->n[0], r, st));
+    CU(pl, launch_mid_passes(pl, f, st));
+    fill_row_args(pl, f, r, nullptr, 0.f, 0);
+    r.p = (float2 *)out;
+    r.V = f.V;  // only multiplies a value that is dropped when do_fwd = 0
+    CU(pl, launch_row<false>(pl->n[0], r, st));
+    CU(pl, cudaStreamSynchronize(st));
+    return TBS_OK;
+}
+
+tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, double tol, int ref_row,
+                                     double surface_pressure_pa, float *p1_out, float *p2_out,
+                                     double *history1, double *history2, int32_t *n_terms1,
+                                     int32_t *n_terms2, void *stream) {
+    if (!p1 || !p2 || p1->fr.size() != 1 || p2->fr.size() != 1 || p1->ndim != p2->ndim) return TBS_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a)
+        if (p1->n[a] != p2->n[a]) return fail(p2, TBS_ERR_INVALID_ARG, "plans differ in grid size");
+    if (fabs(p2->fr[0].f - 2.0 * p1->fr[0].f) > 1e-9 * p1->fr[0].f)
+        return fail(p2, TBS_ERR_INVALID_ARG, "second plan must be created at twice the fundamental");
+    const int nslow = p1->ndim == 2 ? p1->n[1] : p1->n[2];
+    if (ref_row < 0 || ref_row >= nslow) return fail(p1, TBS_ERR_INVALID_ARG, "ref_row outside the grid");
+    cudaStream_t st = (cudaStream_t)stream;
+    tbs_status s1 = solve_all(p1, max_terms, tol, p1_out, false, history1, n_terms1, st);
+    if (s1 < 0) return s1;
+    // S2 = -xi (2 w1)^2 (1/2) p1^2, xi = beta/(rho0 c0^4)  (Eq. 28b)
+    const double xi = p1->beta / (p1->rho0 * pow(p1->c0, 4.0));
+    const double w2 = 2.0 * p1->fr[0].omega;
+    const double coef = -xi * w2 * w2 * 0.5;
+    const long long slab = p1->npts / nslow;
+    cudaMemsetAsync(p1->maxbits, 0, sizeof(unsigned int), st);
+    k_row_max<<<nblk(slab, 256), 256, 0, st>>>(p1->fr[0].p, (long long)ref_row * slab, slab, p1->maxbits);
+    k_second_harmonic_source<<<nblk(p1->npts, 256), 256, 0, st>>>(p1->fr[0].p, p2->fr[0].S, p1->maxbits,
+                                                                   surface_pressure_pa, coef, p1->npts);
+    CU(p1, cudaGetLastError());
+    CU(p1, cudaMemcpyAsync(p1_out, p1->fr[0].p, sizeof(float2) * p1->npts, cudaMemcpyDeviceToDevice, st));
+    p2->fr[0].have_S = true;
+    tbs_status s2 = solve_all(p2, max_terms, tol, p2_out, false, history2, n_terms2, st);
+    p1->launches += 2;
+    return worst(s1, s2);
+}
+
+tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4], void *stream) {
+    if (!pl || !out_ms || reps < 1 || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    Freq &f = pl->fr[ifreq];
+    if (!f.have_V || !f.have_S) return fail(pl, TBS_ERR_NOT_READY, "medium and source required");
+    cudaStream_t st = (cudaStream_t)stream;
+    tbs_status hs = ensure_history(pl, 4);
+    if (hs != TBS_OK) return hs;
+    Ctl *h = pl->h_ctl;
+    memset(&h[0], 0, sizeof(Ctl));
+    h[0].max_terms = 1 << 30;
+    h[0].tol = 0.0;
+    CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
+    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
+    RowArgs r;
+    fill_row_args(pl, f, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row<true>(pl->n[0], r, st));
+    CU(pl, launch_term(pl, f, st));   // warm: p, W hold finite data
+    for (int k = 0; k < 4; ++k) out_ms[k] = 0.0;
+    const int nmid = mid_launches(pl);
+    for (int k = 0; k <= nmid; ++k) {
+        // reset the term counter so the row kernel keeps writing history slot 1
+        CU(pl, cudaEventRecord(pl->ev_t0, st));
+        for (int i = 0; i < reps; ++i) {
+            if (k == 0) {
+                CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
+                fill_row_args(pl, f, r, nullptr, 0.f, 1);
+                CU(pl, launch_row<false>(pl->n[0], r, st));
+            } else {
+                CU(pl, launch_mid_passes(pl, f, st, k - 1));
+            }
+        }
+        CU(pl, cudaEventRecord(pl->ev_t1, st));
+        CU(pl, cudaStreamSynchronize(st));
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, pl->ev_t0, pl->ev_t1);
+        out_ms[k] = ms / reps;
+    }
+    return TBS_OK;
+}
+
+}  // extern "C"

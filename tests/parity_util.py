@@ -1,0 +1,52 @@
+"""Shared helpers for the GPU-vs-oracle parity tests: run one workload through both sides.
+
+The oracle side uses only oracle/tbs_ref.py; the CUDA side only the C-ABI binding.  Both consume
+the same float32 maps from tbs_workloads.py.
+"""
+import numpy as np
+
+import oracle.tbs_ref as R
+
+REL_L2_TOL = 1e-4      # BASELINE.json north_star
+MAX_ABS_TOL = 1e-3     # x max|p|
+
+
+def oracle_run(w, max_terms, tol, ifreq=0, abl_cells=0, S_override=None):
+    f = w.freqs[ifreq]
+    k0, eps = R.wavenumber(f, w.c0, w.damping)
+    g = R.green_spectrum(tuple(2 * s for s in w.shape), w.dx, k0, eps)
+    V = R.potential(w.c.astype(np.float64), w.alpha0_db, w.y, f, w.c0, w.damping)
+    S = S_override if S_override is not None else R.deposit(w.shape, w.dx, w.src_pos, w.src_amp[ifreq])
+    win = None
+    if abl_cells:
+        win = tuple(R.abl_window(n, abl_cells) for n in w.shape[::-1])
+    return R.solve(V, S, g, max_terms, tol, windows=win)
+
+
+def gpu_plan(w, abl_cells=0, graph_batch=None):
+    import torch
+    from paper_2507_13754_b200.tbs import Plan
+    plan = Plan(w.shape, w.dx, w.freqs, w.c0, w.damping)
+    if graph_batch is not None:
+        plan.set_graph_batch(graph_batch)
+    if abl_cells:
+        plan.set_abl(abl_cells)
+    plan.set_medium(torch.from_numpy(w.c).cuda(), alpha0_db=w.alpha0_db, y=w.y, beta=w.beta, rho0=w.rho0)
+    plan.set_source(w.src_pos, w.src_amp)
+    return plan
+
+
+def compare_fields(p_gpu, p_ref, what=""):
+    p_gpu = np.asarray(p_gpu).astype(np.complex128)
+    rel = np.linalg.norm(p_gpu - p_ref) / np.linalg.norm(p_ref)
+    mx = np.abs(p_gpu - p_ref).max() / np.abs(p_ref).max()
+    assert rel <= REL_L2_TOL, f"{what}: rel L2 {rel:.3e} > {REL_L2_TOL}"
+    assert mx <= MAX_ABS_TOL, f"{what}: max |dp| {mx:.3e} x max|p| > {MAX_ABS_TOL}"
+    return rel, mx
+
+
+def compare_history(h_gpu, h_ref, n, rtol=2e-3):
+    h_gpu = np.asarray(h_gpu)[: n + 1]
+    h_ref = np.asarray(h_ref)[: n + 1]
+    assert h_gpu[0] == 1.0
+    assert np.allclose(h_gpu, h_ref, rtol=rtol, atol=0), np.abs(h_gpu / h_ref - 1).max()
