@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py -- Born-series grid-point-terms/s on one B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one synthetic workload: tbs_solve on the
+configuration named in ``config.workload`` (default cfg3, 2-D 2048^2, the size the >=60 % HBM target
+is quoted on), i.e. term 0 plus every Born term until the relative term norm drops below tol.
+  value  = grid points x (terms + 1) x frequencies / device time of the solve, inputs resident in HBM
+  e2e    = the same metric through the C ABI with HOST buffers (medium map and sources copied in,
+           field and history copied out, inside the timed region)
+  roofline     = dominant kernel, algorithmic bytes / CUDA-event duration vs measured HBM copy peak
+  cpu_baseline = the oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
+``--impl reference`` times the oracle instead (bounded sample per step).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import tbs_workloads as W  # noqa: E402
+
+METRIC = "born_series_grid_point_terms_per_sec"
+UNIT = "grid-point-terms/s"
+ALG_BYTES = {2: {"k_row": 56.0, "k_col_conv": 32.0},
+             3: {"k_row": 56.0, "k_col_fwd_y": 48.0, "k_col_conv_z": 64.0, "k_col_inv_y": 48.0}}
+
+
+def make_workload(name):
+    table = {
+        "cfg1": lambda: W.cfg1(), "cfg2": lambda: W.cfg2(), "cfg3": lambda: W.cfg3(), "cfg4": lambda: W.cfg4(),
+        "cfg5": lambda: W.cfg5(), "cfg5_batch16": lambda: W.cfg5(nfreq=16),
+        "cfg3_small": lambda: W.cfg3(N=256),
+    }
+    return table[name]()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(w, terms):
+    """Time the oracle (as it stands) on `terms` Born terms of workload w, frequency 0."""
+    import oracle.tbs_ref as R
+    f = w.freqs[0]
+    k0, eps = R.wavenumber(f, w.c0, w.damping)
+    g = R.green_spectrum(tuple(2 * s for s in w.shape), w.dx, k0, eps)
+    V = R.potential(w.c.astype(np.float64), w.alpha0_db, w.y, f, w.c0, w.damping)
+    S = R.deposit(w.shape, w.dx, w.src_pos, w.src_amp[0])
+    t0 = time.perf_counter()
+    res = R.solve(V, S, g, terms, 0.0)
+    dt = time.perf_counter() - t0
+    return w.n_points * (res.n_terms + 1) / dt, dt, R.num_threads()
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    terms = args.ref_terms
+    vals, times = [], []
+    cores = 0
+    for i in range(args.warmup + args.steps):
+        v, dt, cores = oracle_sample(w, terms)
+        if i >= args.warmup:
+            vals.append(v); times.append(dt)
+    value = w.n_points * (terms + 1) * len(times) / sum(times)
+    sample = f"{terms} Born terms + term 0 of {w.name}, frequency 0, per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex128",
+        "data": "synthetic", "config": {"workload": w.name, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--max-terms", type=int, default=None)
+    ap.add_argument("--tol", type=float, default=None)
+    ap.add_argument("--ref-terms", type=int, default=2, help="Born terms per step of the oracle arm")
+    ap.add_argument("--cpu-baseline-terms", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    w = make_workload(args.workload)
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    import torch
+    from paper_2507_13754_b200.tbs import Plan
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    max_terms = args.max_terms if args.max_terms is not None else w.max_terms
+    tol = args.tol if args.tol is not None else w.tol
+    nf = len(w.freqs)
+
+    plan = Plan(w.shape, w.dx, w.freqs, w.c0, w.damping)
+    c_dev = torch.from_numpy(w.c).cuda()
+    plan.set_medium(c_dev, alpha0_db=w.alpha0_db, y=w.y, beta=w.beta, rho0=w.rho0)
+    plan.set_source(w.src_pos, w.src_amp)
+    p_dev = torch.empty((nf,) + w.shape, dtype=torch.complex64, device="cuda")
+    c_host = torch.from_numpy(w.c).pin_memory()
+    p_host = torch.empty((nf,) + w.shape, dtype=torch.complex64).pin_memory()
+    l2_flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def device_step():
+        l2_flush.zero_()
+        return plan.solve(max_terms, tol, out=p_dev)
+
+    def e2e_step():
+        l2_flush.zero_()
+        plan.set_medium_host(c_host.numpy(), alpha0_db=w.alpha0_db, y=w.y, beta=w.beta, rho0=w.rho0)
+        plan.set_source(w.src_pos, w.src_amp)
+        return plan.solve_host(max_terms, tol, out=p_host.numpy())
+
+    # ---- device-resident arm ----
+    for _ in range(args.warmup):
+        res = device_step()
+    barrier()
+    launches, terms_total, loop_ms = 0, 0, 0.0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            res = device_step()
+            launches += res.launches + 1            # + the L2 flush memset
+            terms_total += int((res.n_terms + 1).sum())
+            loop_ms += res.loop_ms
+        ev1.record()
+        barrier()
+    dt_ms = ev0.elapsed_time(ev1)
+    clocks = clk.summary()
+    status, n_terms = int(res.status), [int(t) for t in res.n_terms]
+
+    # ---- end-to-end arm (host buffers through the C ABI) ----
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_terms = 0
+    for _ in range(args.steps):
+        r2 = e2e_step()
+        e2e_terms += int((r2.n_terms + 1).sum())
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    if dist is not None:
+        t = torch.tensor([dt_ms, e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt_ms, e2e_s = float(t[0]), float(t[1])
+        cnt = torch.tensor([terms_total, e2e_terms, launches], device="cuda", dtype=torch.float64)
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+        terms_total, e2e_terms, launches = (int(v) for v in cnt.tolist())
+
+    value = w.n_points * terms_total / (dt_ms * 1e-3)
+    e2e_value = w.n_points * e2e_terms / e2e_s
+
+    # ---- per-kernel durations (CUDA events on the launching stream) and roofline ----
+    peak, peak_src = measured_peaks()
+    kms = plan.profile_term(0, reps=20)
+    names = list(ALG_BYTES[w.ndim].keys())
+    kernels = []
+    for name, ms in zip(names, kms):
+        b = ALG_BYTES[w.ndim][name] * w.n_points
+        kernels.append({"kernel": name, "ms": float(ms), "alg_bytes": b, "achieved_gbs": b / (ms * 1e-3) / 1e9,
+                        "frac": b / (ms * 1e-3) / 1e9 / peak})
+    dom = max(kernels, key=lambda k: k["ms"])
+    term_ms = loop_ms / max(terms_total / world if world > 1 else terms_total, 1)
+    term_bytes = sum(ALG_BYTES[w.ndim].values()) * w.n_points
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "complex64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": list(w.shape), "padded": [2 * s for s in w.shape],
+                   "frequencies": nf, "tol": tol, "max_terms": max_terms, "n_terms": n_terms,
+                   "solve_status": status, "l2": "256 MiB flush before every step; working set > L2"
+                   if w.n_points * 8 * 4 > 126e6 else "256 MiB flush before every step; working set fits L2",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "time_to_converged_field_ms": dt_ms / args.steps,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT,
+                "h2d_bytes_per_step": int(w.c.nbytes + w.src_pos.nbytes + w.src_amp.nbytes),
+                "d2h_bytes_per_step": int(p_host.numel() * 8 + nf * (max_terms + 1) * 8 + nf * 4),
+                "ms_per_step": 1e3 * e2e_s / args.steps},
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
+                     "unit": "GB/s", "frac": dom["frac"], "traffic": None, "peak_source": peak_src},
+        "kernels": kernels,
+        "term_loop": {"ms_per_term": term_ms, "alg_bytes_per_term": term_bytes,
+                      "achieved_gbs": term_bytes / (term_ms * 1e-3) / 1e9,
+                      "frac_of_hbm_peak": term_bytes / (term_ms * 1e-3) / 1e9 / peak},
+    }
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            v, dt, cores = oracle_sample(w, args.cpu_baseline_terms)
+            out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                   "sample": f"{args.cpu_baseline_terms} Born terms + term 0 of {w.name}, "
+                                             f"frequency 0 ({dt:.1f} s)"}
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

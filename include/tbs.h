@@ -128,9 +128,11 @@ tbs_status tbs_green_spectrum(tbs_plan *plan, int ifreq, float *out, void *strea
  * loop measured with CUDA events on `stream`. */
 int64_t tbs_last_launch_count(const tbs_plan *plan);
 double tbs_last_loop_ms(const tbs_plan *plan);
-/* Per-kernel device time of ONE term (ms) for frequency ifreq, measured with CUDA events around
- * `reps` back-to-back launches of each kernel: out_ms[0..3] = row kernel K31, column/plane
- * passes K2 (2-D) or Ky-fwd, Kz, Ky-inv (3-D: out_ms[1..3]).  Requires medium and source. */
+/* Per-kernel device time of ONE term (ms) for frequency ifreq: runs a live series (term 0, three
+ * warm-up terms, then `reps` <= 256 terms, no graph) with a CUDA event recorded on `stream` between
+ * consecutive kernels, and averages per kernel: out_ms[0] = row kernel K31, out_ms[1] = K2 (2-D) or
+ * out_ms[1..3] = y-forward, z-convolution, y-inverse passes (3-D).  Requires medium and source;
+ * overwrites the plan's running field. */
 tbs_status tbs_profile_term(tbs_plan *plan, int ifreq, int reps, double out_ms[4], void *stream);
 /* Terms per graph launch (default 16); 0 disables CUDA graphs (plain launches). */
 tbs_status tbs_set_graph_batch(tbs_plan *plan, int terms_per_graph);

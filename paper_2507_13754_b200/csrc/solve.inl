@@ -184,12 +184,13 @@ tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, 
 }
 
 tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4], void *stream) {
-    if (!pl || !out_ms || reps < 1 || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    if (!pl || !out_ms || reps < 1 || reps > 256 || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
     Freq &f = pl->fr[ifreq];
     if (!f.have_V || !f.have_S) return fail(pl, TBS_ERR_NOT_READY, "medium and source required");
     cudaStream_t st = (cudaStream_t)stream;
-    tbs_status hs = ensure_history(pl, 4);
+    tbs_status hs = ensure_history(pl, reps + 4);
     if (hs != TBS_OK) return hs;
+    // A real series: term 0, two warm-up terms, then `reps` terms with an event between kernels.
     Ctl *h = pl->h_ctl;
     memset(&h[0], 0, sizeof(Ctl));
     h[0].max_terms = 1 << 30;
@@ -199,27 +200,31 @@ tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4],
     RowArgs r;
     fill_row_args(pl, f, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
     CU(pl, launch_row<true>(pl->n[0], r, st));
-    CU(pl, launch_term(pl, f, st));   // warm: p, W hold finite data
-    for (int k = 0; k < 4; ++k) out_ms[k] = 0.0;
+    for (int i = 0; i < 3; ++i) CU(pl, launch_term(pl, f, st));
     const int nmid = mid_launches(pl);
-    for (int k = 0; k <= nmid; ++k) {
-        // reset the term counter so the row kernel keeps writing history slot 1
-        CU(pl, cudaEventRecord(pl->ev_t0, st));
-        for (int i = 0; i < reps; ++i) {
-            if (k == 0) {
-                CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
-                fill_row_args(pl, f, r, nullptr, 0.f, 1);
-                CU(pl, launch_row<false>(pl->n[0], r, st));
-            } else {
-                CU(pl, launch_mid_passes(pl, f, st, k - 1));
-            }
+    const int per = nmid + 1;
+    std::vector<cudaEvent_t> evs((size_t)reps * per + 1);
+    for (auto &e : evs) CU(pl, cudaEventCreate(&e));
+    fill_row_args(pl, f, r, nullptr, 0.f, 1);
+    CU(pl, cudaEventRecord(evs[0], st));
+    for (int i = 0; i < reps; ++i) {
+        for (int k = 0; k < nmid; ++k) {
+            CU(pl, launch_mid_passes(pl, f, st, k));
+            CU(pl, cudaEventRecord(evs[(size_t)i * per + k + 1], st));
         }
-        CU(pl, cudaEventRecord(pl->ev_t1, st));
-        CU(pl, cudaStreamSynchronize(st));
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, pl->ev_t0, pl->ev_t1);
-        out_ms[k] = ms / reps;
+        CU(pl, launch_row<false>(pl->n[0], r, st));
+        CU(pl, cudaEventRecord(evs[(size_t)i * per + nmid + 1], st));
     }
+    CU(pl, cudaStreamSynchronize(st));
+    for (int k = 0; k < 4; ++k) out_ms[k] = 0.0;
+    for (int i = 0; i < reps; ++i)
+        for (int k = 0; k < per; ++k) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, evs[(size_t)i * per + k], evs[(size_t)i * per + k + 1]);
+            // out_ms[0] = row kernel, out_ms[1..] = column/plane passes in launch order
+            out_ms[k == nmid ? 0 : k + 1] += ms / reps;
+        }
+    for (auto &e : evs) cudaEventDestroy(e);
     return TBS_OK;
 }
 
