@@ -4,18 +4,19 @@
 
 namespace tbs {
 
-// Column-tile kernels: T adjacent lines per CTA, NT threads.  Shared memory = N*T*8 bytes.
+// Column-tile kernels: T adjacent lines per CTA, NT threads.  Shared memory = 2*N*T*8 bytes
+// (both parity halves of the padded line).
 template <int N> struct ColCfg;
 template <> struct ColCfg<32>   { static constexpr int T = 16, NT = 64;  };
 template <> struct ColCfg<64>   { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<128>  { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<256>  { static constexpr int T = 16, NT = 256; };
-template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 256; };
-template <> struct ColCfg<1024> { static constexpr int T = 8,  NT = 256; };
-template <> struct ColCfg<2048> { static constexpr int T = 8,  NT = 512; };
-template <> struct ColCfg<4096> { static constexpr int T = 4,  NT = 512; };
+template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
+template <> struct ColCfg<1024> { static constexpr int T = 8,  NT = 512; };
+template <> struct ColCfg<2048> { static constexpr int T = 4,  NT = 512; };
+template <> struct ColCfg<4096> { static constexpr int T = 2,  NT = 512; };
 
-// Row kernels: ROWS rows per CTA, NT threads.  Shared memory = ROWS*(N + N/16)*8 bytes.
+// Row kernels: ROWS rows per CTA, NT threads.  Shared memory = 2*ROWS*(N + N/16)*8 bytes.
 template <int N> struct RowCfg;
 template <> struct RowCfg<32>   { static constexpr int ROWS = 16, NT = 64;  };
 template <> struct RowCfg<64>   { static constexpr int ROWS = 8,  NT = 64;  };
@@ -29,7 +30,7 @@ template <> struct RowCfg<4096> { static constexpr int ROWS = 1,  NT = 256; };
 template <int N, int MODE>
 static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
     using C = ColCfg<N>;
-    constexpr size_t smem = (size_t)N * C::T * sizeof(float2);
+    constexpr size_t smem = 2 * (size_t)N * C::T * sizeof(float2);
     auto kern = k_col<N, C::T, C::NT, MODE>;
     if (set_attr) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const unsigned grid = (unsigned)(n_outer * (a.inner_len / C::T));
@@ -56,7 +57,7 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
 template <int N, bool FIRST>
 static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
-    constexpr size_t smem = (size_t)C::ROWS * RowLay<N>::PITCH * sizeof(float2);
+    constexpr size_t smem = 2 * (size_t)C::ROWS * RowLay<N>::PITCH * sizeof(float2);
     auto kern = k_row<N, C::ROWS, C::NT, FIRST>;
     if (set_attr) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     kern<<<(unsigned)(a.rows / C::ROWS), C::NT, smem, st>>>(a);

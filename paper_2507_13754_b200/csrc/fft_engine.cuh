@@ -87,6 +87,55 @@ __device__ __forceinline__ void bfly(float2 (&v)[R]) {
     }
 }
 
+// ---- per-stage twiddle look-up tables ---------------------------------------------------------
+// A stage with block length LB = R*S needs w_LB^(k t), k < R, for its sub-index t < S.  The tables
+// are stored [t][R] (float2) so that one thread fetches its R twiddles with R/2 128-bit loads from
+// one contiguous, 16-byte-aligned chunk (built in double by k_stage_lut, setup_kernels.cuh):
+//   lutA[t][k] = w_N^(k t)            first / last stage, even-frequency half (parity 0)
+//   lutB[t][k] = w_2N^((2k+1) t)      first / last stage, odd-frequency half  (parity 1): the
+//                                     zero-padding twist w_2N^(pos), pos = t + j*S1, factors into
+//                                     w_2N^t (folded into the table) and the constant w_(2 R1)^j
+//   lutC[t][k] = w_S1^(k t)           middle stage (three-stage plans only)
+struct Luts {
+    const float2 *A, *B, *C;
+};
+
+template <int R>
+__device__ __forceinline__ void load_tw(float2 (&w)[R], const float2 *__restrict__ lut, int t) {
+    const float4 *p = reinterpret_cast<const float4 *>(lut + (size_t)t * R);
+#pragma unroll
+    for (int i = 0; i < R / 2; ++i) {
+        const float4 v = __ldg(p + i);
+        w[2 * i] = make_float2(v.x, v.y);
+        w[2 * i + 1] = make_float2(v.z, v.w);
+    }
+}
+
+// d * w_32^(idx) with sign SGN; idx in [0, 16).
+template <int SGN>
+__device__ __forceinline__ float2 mul_w32(float2 d, int idx) {
+    constexpr float C[16] = {1.0f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f,
+                             0.70710678118654752f, 0.55557023301960218f, 0.38268343236508977f,
+                             0.19509032201612825f, 0.0f, -0.19509032201612825f, -0.38268343236508977f,
+                             -0.55557023301960218f, -0.70710678118654752f, -0.83146961230254524f,
+                             -0.92387953251128674f, -0.98078528040323043f};
+    constexpr float S[16] = {0.0f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f,
+                             0.70710678118654752f, 0.83146961230254524f, 0.92387953251128674f,
+                             0.98078528040323043f, 1.0f, 0.98078528040323043f, 0.92387953251128674f,
+                             0.83146961230254524f, 0.70710678118654752f, 0.55557023301960218f,
+                             0.38268343236508977f, 0.19509032201612825f};
+    if (idx == 0) return d;
+    if (idx == 8) return make_float2(-(float)SGN * d.y, (float)SGN * d.x);
+    const float c = C[idx], s = (float)SGN * S[idx];
+    return make_float2(d.x * c - d.y * s, d.y * c + d.x * s);
+}
+// x[j] *= w_(2R)^(SGN j): the constant part of the zero-padding twist of the odd-frequency half.
+template <int R, int SGN>
+__device__ __forceinline__ void twist_const(float2 (&x)[R]) {
+#pragma unroll
+    for (int j = 1; j < R; ++j) x[j] = mul_w32<SGN>(x[j], j * (16 / R));
+}
+
 // ---- shared-memory layouts -------------------------------------------------------------------
 // Column tile: T adjacent lines interleaved, [pos][T].  A warp covers 32/T positions x T lines.
 // XOR swizzle of the low position bits keeps the contiguous-block stage (stride RL between
@@ -112,11 +161,13 @@ struct RowLay {
     __device__ static __forceinline__ void split(int w, int &line, int &b) { b = w % NBL; line = w / NBL; }
 };
 
-// ---- generic in-place stage on shared memory ---------------------------------------------------
-// Block length LB, radix R, sub-stride S = LB/R.  DIF: butterfly then twiddle w_LB^(k t);
-// DIT (inverse): conj twiddle then butterfly.  `total` = number of butterflies in the tile.
-template <int N, int LB, int R, bool FWD, class Lay, int NT>
-__device__ __forceinline__ void stage_smem(float2 *sm, const float2 *__restrict__ tw, int tid, int total) {
+// ---- in-place stages on shared memory, both parity halves at once --------------------------------
+// sm holds the even-frequency half at [0, HALF) and the odd-frequency half at [HALF, 2 HALF); one
+// work item is the pair of butterflies (parity 0, parity 1) at the same (line, block, t), which
+// share their twiddles.  Block length LB, radix R, sub-stride S = LB/R.
+// FWD (DIF): butterfly then twiddle w_LB^(k t);  inverse (DIT): conj twiddle then butterfly.
+template <int N, int LB, int R, bool FWD, class Lay, int NT, int HALF>
+__device__ __forceinline__ void stage_pair(float2 *sm, const float2 *__restrict__ lut, int tid, int total) {
     constexpr int S = LB / R;
     constexpr int NBL = N / R;
     for (int w = tid; w < total; w += NT) {
@@ -124,93 +175,141 @@ __device__ __forceinline__ void stage_smem(float2 *sm, const float2 *__restrict_
         Lay::template split<NBL>(w, line, b);
         const int t = b % S;
         const int base = (b / S) * LB + t;
-        float2 v[R];
-        if (FWD) {
+        float2 tw[R];
+        if (S > 1) load_tw<R>(tw, lut, t);
 #pragma unroll
-            for (int j = 0; j < R; ++j) v[j] = sm[Lay::addr(line, base + j * S)];
-            bfly<R, -1>(v);
+        for (int p = 0; p < 2; ++p) {
+            float2 *s = sm + p * HALF;
+            float2 v[R];
+            if (FWD) {
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-                const int k = brev(i, R);
-                float2 o = v[i];
-                if (S > 1 && k > 0) o = cmul(o, __ldg(&tw[k * t * (NTW / LB)]));
-                sm[Lay::addr(line, base + k * S)] = o;
+                for (int j = 0; j < R; ++j) v[j] = s[Lay::addr(line, base + j * S)];
+                bfly<R, -1>(v);
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const int k = brev(i, R);
+                    float2 o = v[i];
+                    if (S > 1 && k > 0) o = cmul(o, tw[k]);
+                    s[Lay::addr(line, base + k * S)] = o;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < R; ++k) {
+                    float2 x = s[Lay::addr(line, base + k * S)];
+                    if (S > 1 && k > 0) x = cmulc(x, tw[k]);
+                    v[k] = x;
+                }
+                bfly<R, +1>(v);
+#pragma unroll
+                for (int i = 0; i < R; ++i) s[Lay::addr(line, base + brev(i, R) * S)] = v[i];
             }
-        } else {
-#pragma unroll
-            for (int k = 0; k < R; ++k) {
-                float2 x = sm[Lay::addr(line, base + k * S)];
-                if (S > 1 && k > 0) x = cmulc(x, __ldg(&tw[k * t * (NTW / LB)]));
-                v[k] = x;
-            }
-            bfly<R, +1>(v);
-#pragma unroll
-            for (int i = 0; i < R; ++i) sm[Lay::addr(line, base + brev(i, R) * S)] = v[i];
         }
     }
 }
 
-// First forward stage from registers: x[j] sits at position t + j*S1 (natural order).
-template <int N, int R1, class Lay>
-__device__ __forceinline__ void first_fwd(float2 (&x)[R1], int line, int t, float2 *sm,
-                                          const float2 *__restrict__ tw) {
+// First forward stage from registers: x[j] is the input at position t + j*S1 (natural order).
+// Writes the even-frequency half (FFT of x) and the odd-frequency half (FFT of x w_2N^pos).
+template <int N, int R1, class Lay, int HALF>
+__device__ __forceinline__ void first_fwd_pair(const float2 (&x)[R1], int line, int t, float2 *sm,
+                                               const Luts &L) {
     constexpr int S1 = N / R1;
-    bfly<R1, -1>(x);
+    float2 tw[R1];
+    float2 v[R1];
+    load_tw<R1>(tw, L.A, t);
+#pragma unroll
+    for (int j = 0; j < R1; ++j) v[j] = x[j];
+    bfly<R1, -1>(v);
 #pragma unroll
     for (int i = 0; i < R1; ++i) {
         const int k = brev(i, R1);
-        float2 o = x[i];
-        if (k > 0) o = cmul(o, __ldg(&tw[k * t * (NTW / N)]));
-        sm[Lay::addr(line, t + k * S1)] = o;
+        sm[Lay::addr(line, t + k * S1)] = k > 0 ? cmul(v[i], tw[k]) : v[i];
+    }
+    load_tw<R1>(tw, L.B, t);
+#pragma unroll
+    for (int j = 0; j < R1; ++j) v[j] = x[j];
+    twist_const<R1, -1>(v);
+    bfly<R1, -1>(v);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) {
+        const int k = brev(i, R1);
+        sm[HALF + Lay::addr(line, t + k * S1)] = cmul(v[i], tw[k]);
     }
 }
 
-// Last inverse stage into registers: z[j] is the (unnormalised) inverse at position t + j*S1.
-template <int N, int R1, class Lay>
-__device__ __forceinline__ void last_inv(float2 (&z)[R1], int line, int t, const float2 *sm,
-                                         const float2 *__restrict__ tw) {
+// Last inverse stage into registers, both halves combined (inverse of first_fwd_pair followed by
+// the crop): z[j] = IFFT_N(even half)[pos] + conj(w_2N^pos) IFFT_N(odd half)[pos], pos = t + j*S1.
+template <int N, int R1, class Lay, int HALF>
+__device__ __forceinline__ void last_inv_pair(float2 (&z)[R1], int line, int t, const float2 *sm,
+                                              const Luts &L) {
     constexpr int S1 = N / R1;
-    float2 v[R1];
+    float2 tw[R1];
+    float2 v[R1], u[R1];
+    load_tw<R1>(tw, L.A, t);
 #pragma unroll
     for (int k = 0; k < R1; ++k) {
-        float2 x = sm[Lay::addr(line, t + k * S1)];
-        if (k > 0) x = cmulc(x, __ldg(&tw[k * t * (NTW / N)]));
-        v[k] = x;
+        const float2 a = sm[Lay::addr(line, t + k * S1)];
+        v[k] = k > 0 ? cmulc(a, tw[k]) : a;
     }
     bfly<R1, +1>(v);
+    load_tw<R1>(tw, L.B, t);
 #pragma unroll
-    for (int i = 0; i < R1; ++i) z[brev(i, R1)] = v[i];
+    for (int k = 0; k < R1; ++k) u[k] = cmulc(sm[HALF + Lay::addr(line, t + k * S1)], tw[k]);
+    bfly<R1, +1>(u);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) {
+        const int j = brev(i, R1);
+        z[j] = cadd(v[i], mul_w32<+1>(u[i], j * (16 / R1)));
+    }
+}
+
+// 1/d to ~1 ulp without the IEEE-division slow path: MUFU.RCP + one Newton step.  d >= e^2 > 0.
+__device__ __forceinline__ float rcp_nr(float d) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d));
+    return fmaf(r, fmaf(-d, r, 1.0f), r);
 }
 
 // Fused middle of the convolution: last forward stage (contiguous blocks of RL), multiply by
 // ghat, first inverse stage -- all in registers (north_star: "pointwise G multiply fused into the
 // last forward and first inverse butterfly stage").
 //   ghat' = scale / (a - i e),  a = a_line + p2[P],  e = eps/k0^2   (non-dimensional)
-template <int N, int RL, class Lay, int NT>
-__device__ __forceinline__ void mid_conv(float2 *sm, int tid, int total, const float *__restrict__ p2half,
-                                         float a_line, float e, float scale) {
+template <int N, int RL, class Lay, int NT, int HALF>
+__device__ __forceinline__ void mid_conv_pair(float2 *sm, int tid, int total, const float *__restrict__ p2line,
+                                              float a_line, float e, float scale) {
     constexpr int NBL = N / RL;
     const float e2 = e * e;
     for (int w = tid; w < total; w += NT) {
         int line, b;
         Lay::template split<NBL>(w, line, b);
         const int base = b * RL;
-        float2 v[RL];
 #pragma unroll
-        for (int j = 0; j < RL; ++j) v[j] = sm[Lay::addr(line, base + j)];
-        bfly<RL, -1>(v);
-        float2 u[RL];
+        for (int p = 0; p < 2; ++p) {
+            float2 *s = sm + p * HALF;
+            float2 v[RL];
+            float pp[RL];
+            // RL consecutive table entries, 16-byte aligned
+            const float4 *pt = reinterpret_cast<const float4 *>(p2line + p * N + base);
 #pragma unroll
-        for (int i = 0; i < RL; ++i) {
-            const int k = brev(i, RL);
-            const float a = a_line + __ldg(&p2half[base + k]);
-            const float r = __fdiv_rn(scale, fmaf(a, a, e2));
-            const float gr = a * r, gi = e * r;
-            u[k] = make_float2(v[i].x * gr - v[i].y * gi, v[i].x * gi + v[i].y * gr);
+            for (int q = 0; q < RL / 4; ++q) {
+                const float4 f = __ldg(pt + q);
+                pp[4 * q] = f.x; pp[4 * q + 1] = f.y; pp[4 * q + 2] = f.z; pp[4 * q + 3] = f.w;
+            }
+#pragma unroll
+            for (int j = 0; j < RL; ++j) v[j] = s[Lay::addr(line, base + j)];
+            bfly<RL, -1>(v);
+            float2 u[RL];
+#pragma unroll
+            for (int i = 0; i < RL; ++i) {
+                const int k = brev(i, RL);
+                const float a = a_line + pp[k];
+                const float r = scale * rcp_nr(fmaf(a, a, e2));
+                const float gr = a * r, gi = e * r;
+                u[k] = make_float2(v[i].x * gr - v[i].y * gi, v[i].x * gi + v[i].y * gr);
+            }
+            bfly<RL, +1>(u);
+#pragma unroll
+            for (int i = 0; i < RL; ++i) s[Lay::addr(line, base + brev(i, RL))] = u[i];
         }
-        bfly<RL, +1>(u);
-#pragma unroll
-        for (int i = 0; i < RL; ++i) sm[Lay::addr(line, base + brev(i, RL))] = u[i];
     }
 }
 

@@ -9,6 +9,8 @@
 //          CONV: pad, FFT, .ghat, IFFT, crop, in place   (K2 in 2-D, the z pass in 3-D)
 //          FWD : pad, FFT  N -> 2N positions             (3-D y pass, forward)
 //          INV : IFFT, crop  2N positions -> N           (3-D y pass, inverse)
+// Both parity halves of a padded line (fft_engine.cuh) are resident in shared memory at once, so
+// the input is read once and the twiddles of a butterfly pair are fetched once.
 #pragma once
 #include "fft_engine.cuh"
 
@@ -37,7 +39,7 @@ struct ColArgs {
     const float *p2_inner;  // [inner_len] of the inner (x) axis, position order  (CONV)
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
     float e, scale;         // eps/k0^2 and 1/prod(2N)                            (CONV)
-    const float2 *tw;
+    Luts lut;
     const Ctl *ctl;
 };
 
@@ -45,11 +47,12 @@ template <int N, int T, int NT, int MODE>
 __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
+    constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
     static_assert((S1 * T) % NT == 0 && NT % T == 0, "tile/thread mismatch");
-    constexpr int NB = (S1 * T) / NT;  // first/last-stage butterflies per thread
+    constexpr int NB = (S1 * T) / NT;  // first/last-stage butterfly pairs per thread
     constexpr int TSTEP = NT / T;
-    constexpr int M = 2 * N;
+    constexpr int HALF = N * T;
     using Lay = ColLay<N, T, RL>;
     extern __shared__ float2 sm[];
     if (a.ctl->done) return;
@@ -61,98 +64,72 @@ __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     const int outer = blockIdx.x / tiles;
     const float2 *in = a.in + (long long)outer * a.in_outer_stride + inner0 + line;
     float2 *out = a.out + (long long)outer * a.out_outer_stride + inner0 + line;
-    const float2 *__restrict__ tw = a.tw;
 
-    float a_line = 0.f;
-    if (MODE == MODE_CONV) {
-        a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
-        if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
-    }
-
-    float2 acc[NB][R1];
+    // ---- forward: N inputs -> both halves in smem ----
+    if (MODE != MODE_INV) {
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-        // ---- forward half: N inputs (twisted for s = 1) -> smem, or (INV) load positions ----
-        if (MODE != MODE_INV) {
+        for (int i = 0; i < NB; ++i) {
+            const int t = t0 + i * TSTEP;
+            float2 x[R1];
 #pragma unroll
-            for (int i = 0; i < NB; ++i) {
-                const int t = t0 + i * TSTEP;
-                float2 x[R1];
-#pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    const int pos = t + j * S1;
-                    float2 v = in[(long long)pos * a.in_line_stride];
-                    if (s) v = cmul(v, __ldg(&tw[pos * (NTW / M)]));
-                    x[j] = v;
-                }
-                first_fwd<N, R1, Lay>(x, line, t, sm, tw);
-            }
-            __syncthreads();
-            if (R2 > 0) {
-                stage_smem<N, S1, (R2 > 0 ? R2 : 2), true, Lay, NT>(sm, tw, tid, (N / (R2 > 0 ? R2 : 2)) * T);
-                __syncthreads();
-            }
+            for (int j = 0; j < R1; ++j) x[j] = in[(long long)(t + j * S1) * a.in_line_stride];
+            first_fwd_pair<N, R1, Lay, HALF>(x, line, t, sm, a.lut);
         }
-        if (MODE == MODE_CONV) {
-            mid_conv<N, RL, Lay, NT>(sm, tid, (N / RL) * T, a.p2_line + s * N, a_line, a.e, a.scale);
+        __syncthreads();
+        if (R2 > 0) {
+            stage_pair<N, S1, R2s, true, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
             __syncthreads();
-        } else if (MODE == MODE_FWD) {
-            // last forward stage straight to global: positions s*N + b*RL + k
-            for (int w = tid; w < (N / RL) * T; w += NT) {
-                const int b = w / T;
+        }
+    }
+    if (MODE == MODE_CONV) {
+        float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
+        if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
+        mid_conv_pair<N, RL, Lay, NT, HALF>(sm, tid, (N / RL) * T, a.p2_line, a_line, a.e, a.scale);
+        __syncthreads();
+    } else if (MODE == MODE_FWD) {
+        // last forward stage straight to global: positions s*N + b*RL + k
+        for (int w = tid; w < (N / RL) * T; w += NT) {
+            const int b = w / T;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
                 float2 v[RL];
 #pragma unroll
-                for (int j = 0; j < RL; ++j) v[j] = sm[Lay::addr(line, b * RL + j)];
+                for (int j = 0; j < RL; ++j) v[j] = sm[s * HALF + Lay::addr(line, b * RL + j)];
                 bfly<RL, -1>(v);
 #pragma unroll
                 for (int i = 0; i < RL; ++i)
                     out[(long long)(s * N + b * RL + brev(i, RL)) * a.out_line_stride] = v[i];
             }
-            __syncthreads();
-        } else {
-            // INV: first inverse stage straight from global
-            for (int w = tid; w < (N / RL) * T; w += NT) {
-                const int b = w / T;
+        }
+        return;
+    } else {
+        // INV: first inverse stage straight from global
+        for (int w = tid; w < (N / RL) * T; w += NT) {
+            const int b = w / T;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
                 float2 v[RL];
 #pragma unroll
                 for (int k = 0; k < RL; ++k) v[k] = in[(long long)(s * N + b * RL + k) * a.in_line_stride];
                 bfly<RL, +1>(v);
 #pragma unroll
-                for (int i = 0; i < RL; ++i) sm[Lay::addr(line, b * RL + brev(i, RL))] = v[i];
+                for (int i = 0; i < RL; ++i) sm[s * HALF + Lay::addr(line, b * RL + brev(i, RL))] = v[i];
             }
-            __syncthreads();
         }
-        // ---- inverse half ----
-        if (MODE != MODE_FWD) {
-            if (R2 > 0) {
-                stage_smem<N, S1, (R2 > 0 ? R2 : 2), false, Lay, NT>(sm, tw, tid, (N / (R2 > 0 ? R2 : 2)) * T);
-                __syncthreads();
-            }
-#pragma unroll
-            for (int i = 0; i < NB; ++i) {
-                const int t = t0 + i * TSTEP;
-                float2 z[R1];
-                last_inv<N, R1, Lay>(z, line, t, sm, tw);
-#pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    if (s == 0) acc[i][j] = z[j];
-                    else acc[i][j] = cadd(acc[i][j], cmulc(z[j], __ldg(&tw[(t + j * S1) * (NTW / M)])));
-                }
-            }
-            __syncthreads();
-        }
+        __syncthreads();
     }
-    if (MODE != MODE_FWD) {
+    // ---- inverse: both halves -> N outputs ----
+    if (R2 > 0) {
+        stage_pair<N, S1, R2s, false, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
+        __syncthreads();
+    }
 #pragma unroll
-        for (int i = 0; i < NB; ++i) {
-            const int t = t0 + i * TSTEP;
+    for (int i = 0; i < NB; ++i) {
+        const int t = t0 + i * TSTEP;
+        float2 z[R1];
+        last_inv_pair<N, R1, Lay, HALF>(z, line, t, sm, a.lut);
 #pragma unroll
-            for (int j = 0; j < R1; ++j) {
-                float2 v = acc[i][j];
-                if (MODE == MODE_INV) { v.x *= a.scale; v.y *= a.scale; }
-                out[(long long)(t + j * S1) * a.out_line_stride] = v;
-            }
-        }
+        for (int j = 0; j < R1; ++j) out[(long long)(t + j * S1) * a.out_line_stride] = z[j];
     }
 }
 
@@ -171,8 +148,20 @@ struct RowArgs {
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
     Ctl *ctl;
-    const float2 *tw;
+    Luts lut;
 };
+
+// RL contiguous complex values <-> registers with 128-bit accesses (RL*8 bytes, 16-byte aligned).
+template <int RL>
+__device__ __forceinline__ void load_chunk(float2 (&v)[RL], const float2 *g) {
+    const float4 *p = reinterpret_cast<const float4 *>(g);
+#pragma unroll
+    for (int q = 0; q < RL / 2; ++q) {
+        const float4 f = p[q];
+        v[2 * q] = make_float2(f.x, f.y);
+        v[2 * q + 1] = make_float2(f.z, f.w);
+    }
+}
 
 // FIRST = true : forward half only, w = src * src_scale (term 0: u_0 = G S, Eq. 20)
 // FIRST = false: inverse half (K3) + forward half (K1) of the next term
@@ -180,56 +169,49 @@ template <int N, int ROWS, int NT, bool FIRST>
 __global__ void __launch_bounds__(NT) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
+    constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
     static_assert((ROWS * S1) % NT == 0, "tile/thread mismatch");
     constexpr int NB = (ROWS * S1) / NT;
     constexpr int M = 2 * N;
     using Lay = RowLay<N>;
+    constexpr int HALF = ROWS * Lay::PITCH;
     extern __shared__ float2 sm[];
     __shared__ float red[2][32];
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
     const int row0 = blockIdx.x * ROWS;
-    const float2 *__restrict__ tw = a.tw;
     float2 x[NB][R1];
     const int term = FIRST ? 0 : a.ctl->term;
 
     if (!FIRST) {
         // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
+        // first inverse stage (contiguous blocks of RL) straight from global memory
+        for (int w = tid; w < ROWS * (N / RL); w += NT) {
+            const int b = w % (N / RL), l = w / (N / RL);
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            for (int e = tid; e < ROWS * N; e += NT) {
-                const int l = e / N, pos = e % N;
-                sm[Lay::addr(l, pos)] = a.W[(long long)(row0 + l) * M + s * N + pos];
-            }
-            __syncthreads();
-            stage_smem<N, RL, RL, false, Lay, NT>(sm, tw, tid, ROWS * (N / RL));
-            __syncthreads();
-            if (R2 > 0) {
-                stage_smem<N, S1, (R2 > 0 ? R2 : 2), false, Lay, NT>(sm, tw, tid, ROWS * (N / (R2 > 0 ? R2 : 2)));
-                __syncthreads();
-            }
+            for (int s = 0; s < 2; ++s) {
+                float2 v[RL];
+                load_chunk<RL>(v, a.W + (long long)(row0 + l) * M + s * N + b * RL);
+                bfly<RL, +1>(v);
 #pragma unroll
-            for (int i = 0; i < NB; ++i) {
-                const int w = tid + i * NT;
-                const int t = w % S1, l = w / S1;
-                float2 z[R1];
-                last_inv<N, R1, Lay>(z, l, t, sm, tw);
-#pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    if (s == 0) x[i][j] = z[j];
-                    else x[i][j] = cadd(x[i][j], cmulc(z[j], __ldg(&tw[(t + j * S1) * (NTW / M)])));
-                }
+                for (int i = 0; i < RL; ++i) sm[s * HALF + Lay::addr(l, b * RL + brev(i, RL))] = v[i];
             }
+        }
+        __syncthreads();
+        if (R2 > 0) {
+            stage_pair<N, S1, R2s, false, Lay, NT, HALF>(sm, a.lut.C, tid, ROWS * (N / R2s));
             __syncthreads();
         }
-        // u = A . crop(...);  p (+)= u;  norms;  w = V . u
+        // last inverse stage + crop + window + accumulate; the same thread later writes the same
+        // smem slots in the forward half, so no barrier is needed in between
         float uu = 0.f, pp = 0.f;
 #pragma unroll
         for (int i = 0; i < NB; ++i) {
             const int w = tid + i * NT;
             const int t = w % S1, l = w / S1;
+            last_inv_pair<N, R1, Lay, HALF>(x[i], l, t, sm, a.lut);
             const int row = row0 + l;
             float wrow = __ldg(&a.ay[row % a.ny]);
             if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
@@ -272,9 +254,8 @@ __global__ void __launch_bounds__(NT) k_row(RowArgs a) {
                 a.ctl->ticket = 0;
                 a.ctl->n_terms = term;
                 a.ctl->term = term + 1;
-                if (!(r == r) || r > 1.0e300 || !(np > 0.0 || nu == 0.0)) {
-                    if (!(nu == 0.0 && np == 0.0)) { a.ctl->done = 1; a.ctl->status = -5; }
-                    else { a.ctl->done = 1; a.ctl->status = 0; }
+                if (!(r == r) || r > 1.0e300) {
+                    a.ctl->done = 1; a.ctl->status = -5;
                 } else if (term >= 1 && r < a.ctl->tol) {
                     a.ctl->done = 1; a.ctl->status = 0;
                 } else if (term >= a.ctl->max_terms) {
@@ -298,31 +279,33 @@ __global__ void __launch_bounds__(NT) k_row(RowArgs a) {
 
     // ---------------- forward half: zero-pad (two parity halves), FFT_x ----------------
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
+    for (int i = 0; i < NB; ++i) {
+        const int w = tid + i * NT;
+        const int t = w % S1, l = w / S1;
+        first_fwd_pair<N, R1, Lay, HALF>(x[i], l, t, sm, a.lut);
+    }
+    __syncthreads();
+    if (R2 > 0) {
+        stage_pair<N, S1, R2s, true, Lay, NT, HALF>(sm, a.lut.C, tid, ROWS * (N / R2s));
+        __syncthreads();
+    }
+    // last forward stage (contiguous blocks of RL) straight to global memory
+    for (int w = tid; w < ROWS * (N / RL); w += NT) {
+        const int b = w % (N / RL), l = w / (N / RL);
 #pragma unroll
-        for (int i = 0; i < NB; ++i) {
-            const int w = tid + i * NT;
-            const int t = w % S1, l = w / S1;
-            float2 y[R1];
+        for (int s = 0; s < 2; ++s) {
+            float2 v[RL];
 #pragma unroll
-            for (int j = 0; j < R1; ++j) {
-                y[j] = x[i][j];
-                if (s) y[j] = cmul(y[j], __ldg(&tw[(t + j * S1) * (NTW / M)]));
-            }
-            first_fwd<N, R1, Lay>(y, l, t, sm, tw);
+            for (int j = 0; j < RL; ++j) v[j] = sm[s * HALF + Lay::addr(l, b * RL + j)];
+            bfly<RL, -1>(v);
+            // v[i] = X[brev(i)]: gather into natural order and store 2 values per 128-bit write
+            float2 o[RL];
+#pragma unroll
+            for (int i = 0; i < RL; ++i) o[brev(i, RL)] = v[i];
+            float4 *g = reinterpret_cast<float4 *>(a.W + (long long)(row0 + l) * M + s * N + b * RL);
+#pragma unroll
+            for (int q = 0; q < RL / 2; ++q) g[q] = make_float4(o[2 * q].x, o[2 * q].y, o[2 * q + 1].x, o[2 * q + 1].y);
         }
-        __syncthreads();
-        if (R2 > 0) {
-            stage_smem<N, S1, (R2 > 0 ? R2 : 2), true, Lay, NT>(sm, tw, tid, ROWS * (N / (R2 > 0 ? R2 : 2)));
-            __syncthreads();
-        }
-        stage_smem<N, RL, RL, true, Lay, NT>(sm, tw, tid, ROWS * (N / RL));
-        __syncthreads();
-        for (int e = tid; e < ROWS * N; e += NT) {
-            const int l = e / N, pos = e % N;
-            a.W[(long long)(row0 + l) * M + s * N + pos] = sm[Lay::addr(l, pos)];
-        }
-        __syncthreads();
     }
 }
 

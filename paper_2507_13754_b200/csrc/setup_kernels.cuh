@@ -5,13 +5,19 @@
 
 namespace tbs {
 
-// tw[k] = exp(-2 pi i k / NTW)
-__global__ void k_twiddles(float2 *tw) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= NTW) return;
+// Per-stage twiddle tables (fft_engine.cuh "Luts"), evaluated in double:
+//   which = 0: lut[t][k] = exp(-2 pi i k t / L)            (L = N: table A;  L = S1: table C)
+//   which = 1: lut[t][k] = exp(-2 pi i (2k+1) t / (2 L))   (L = N: table B)
+// t < S = L / R, k < R.
+__global__ void k_stage_lut(float2 *lut, int L, int R, int which) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int S = L / R;
+    if (i >= S * R) return;
+    const int t = i / R, k = i % R;
     double s, c;
-    sincospi(-2.0 * (double)k / (double)NTW, &s, &c);
-    tw[k] = make_float2((float)c, (float)s);
+    if (which == 0) sincospi(-2.0 * (double)((long long)k * t % L) / (double)L, &s, &c);
+    else sincospi(-2.0 * (double)((long long)(2 * k + 1) * t % (2 * L)) / (double)(2 * L), &s, &c);
+    lut[i] = make_float2((float)c, (float)s);
 }
 
 // Frequency index held at `pos` of a length-N DIF transform with radices r1, r2 (0 = none), rl.

@@ -39,7 +39,9 @@ struct tbs_plan {
     double dx = 0, c0 = 0, damping = 0;
     double beta = 1.0, rho0 = 1000.0;
     std::vector<Freq> fr;
-    float2 *tw = nullptr;
+    float2 *lutA[3] = {nullptr, nullptr, nullptr};   // per axis, fft_engine.cuh "Luts"
+    float2 *lutB[3] = {nullptr, nullptr, nullptr};
+    float2 *lutC[3] = {nullptr, nullptr, nullptr};
     float2 *W1 = nullptr;   // [nz*ny][2 nx]
     float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]
     float *abl[3] = {nullptr, nullptr, nullptr};
@@ -103,7 +105,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.norms = pl->norms;
     a.history = pl->history;
     a.ctl = f.ctl;
-    a.tw = pl->tw;
+    a.lut = Luts{pl->lutA[0], pl->lutB[0], pl->lutC[0]};
 }
 
 // Column / plane passes of one term (K2 in 2-D; y-forward, z-conv, y-inverse in 3-D).
@@ -112,13 +114,13 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     const long long mx = 2LL * nx, my = 2LL * ny;
     ColArgs a;
     memset(&a, 0, sizeof a);
-    a.tw = pl->tw;
     a.ctl = f.ctl;
     a.e = (float)pl->damping;
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
         a.in = pl->W1; a.out = pl->W1;
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
         a.in_line_stride = a.out_line_stride = mx;
         a.p2_line = f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
         a.scale = (float)(1.0 / ((double)mx * (double)my));
@@ -129,6 +131,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
     if (which < 0 || which == 0) {
         a.in = pl->W1; a.out = pl->W2;
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = (long long)ny * mx; a.out_outer_stride = my * mx;
         a.scale = 1.f;
@@ -138,6 +141,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     // z convolution, in place on W2; lines (ky, kx), outer = ky
     if (which < 0 || which == 1) {
         a.in = pl->W2; a.out = pl->W2;
+        a.lut = Luts{pl->lutA[2], pl->lutB[2], pl->lutC[2]};
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
         a.p2_line = f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
@@ -148,6 +152,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
     if (which < 0 || which == 2) {
         a.in = pl->W2; a.out = pl->W1;
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = my * mx; a.out_outer_stride = (long long)ny * mx;
         a.p2_line = nullptr; a.p2_inner = nullptr; a.p2_outer = nullptr;
@@ -226,7 +231,8 @@ void tbs_plan_destroy(tbs_plan *pl) {
         cudaFree(f.V); cudaFree(f.S); cudaFree(f.p); cudaFree(f.ctl);
         for (int a = 0; a < 3; ++a) cudaFree(f.p2[a]);
     }
-    cudaFree(pl->tw); cudaFree(pl->W1); cudaFree(pl->W2);
+    for (int a = 0; a < 3; ++a) { cudaFree(pl->lutA[a]); cudaFree(pl->lutB[a]); cudaFree(pl->lutC[a]); }
+    cudaFree(pl->W1); cudaFree(pl->W2);
     for (int a = 0; a < 3; ++a) cudaFree(pl->abl[a]);
     cudaFree(pl->norms); cudaFree(pl->history); cudaFree(pl->maxbits);
     if (pl->h_ctl) cudaFreeHost(pl->h_ctl);
@@ -260,8 +266,19 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
     tbs_status st = TBS_OK;
     auto build = [&]() -> tbs_status {
         CU(pl, set_kernel_attrs(pl));
-        CU(pl, dmalloc(pl, &pl->tw, NTW));
-        k_twiddles<<<nblk(NTW, 256), 256>>>(pl->tw);
+        for (int a = 0; a < ndim; ++a) {
+            int r1, r2, rl;
+            radices_of(pl->n[a], r1, r2, rl);
+            const int N = pl->n[a];
+            CU(pl, dmalloc(pl, &pl->lutA[a], N));
+            CU(pl, dmalloc(pl, &pl->lutB[a], N));
+            k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutA[a], N, r1, 0);
+            k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutB[a], N, r1, 1);
+            if (r2 > 0) {
+                CU(pl, dmalloc(pl, &pl->lutC[a], N / r1));
+                k_stage_lut<<<nblk(N / r1, 256), 256>>>(pl->lutC[a], N / r1, r2, 0);
+            }
+        }
         const long long rows = (long long)pl->n[1] * pl->n[2];
         CU(pl, dmalloc(pl, &pl->W1, (size_t)(rows * 2 * pl->n[0])));
         if (ndim == 3) CU(pl, dmalloc(pl, &pl->W2, (size_t)((long long)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0])));
