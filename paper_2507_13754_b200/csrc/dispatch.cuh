@@ -13,19 +13,30 @@ template <> struct ColCfg<128>  { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<256>  { static constexpr int T = 16, NT = 256; };
 template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
 template <> struct ColCfg<1024> { static constexpr int T = 8,  NT = 512; };
-template <> struct ColCfg<2048> { static constexpr int T = 4,  NT = 512; };
+#ifndef TBS_COL2048_T
+#define TBS_COL2048_T 4
+#define TBS_COL2048_NT 512
+#endif
+template <int T_, int NT_> struct ColCfgT { static constexpr int T = T_, NT = NT_; };
+template <> struct ColCfg<2048> : ColCfgT<TBS_COL2048_T, TBS_COL2048_NT> {};
 template <> struct ColCfg<4096> { static constexpr int T = 2,  NT = 512; };
 
 // Row kernels: ROWS rows per CTA, NT threads.  Shared memory = 2*ROWS*(N + N/16)*8 bytes.
 template <int N> struct RowCfg;
-template <> struct RowCfg<32>   { static constexpr int ROWS = 16, NT = 64;  };
-template <> struct RowCfg<64>   { static constexpr int ROWS = 8,  NT = 64;  };
-template <> struct RowCfg<128>  { static constexpr int ROWS = 8,  NT = 64;  };
-template <> struct RowCfg<256>  { static constexpr int ROWS = 4,  NT = 64;  };
-template <> struct RowCfg<512>  { static constexpr int ROWS = 2,  NT = 128; };
-template <> struct RowCfg<1024> { static constexpr int ROWS = 2,  NT = 128; };
-template <> struct RowCfg<2048> { static constexpr int ROWS = 2,  NT = 256; };
-template <> struct RowCfg<4096> { static constexpr int ROWS = 1,  NT = 256; };
+template <> struct RowCfg<32> { static constexpr int ROWS = 16, NT = 64, MINB = 4; };
+template <> struct RowCfg<64> { static constexpr int ROWS = 8, NT = 64, MINB = 4; };
+template <> struct RowCfg<128> { static constexpr int ROWS = 8, NT = 64, MINB = 4; };
+template <> struct RowCfg<256> { static constexpr int ROWS = 4, NT = 64, MINB = 4; };
+template <> struct RowCfg<512> { static constexpr int ROWS = 2, NT = 128, MINB = 4; };
+template <> struct RowCfg<1024> { static constexpr int ROWS = 2, NT = 128, MINB = 3; };
+#ifndef TBS_ROW2048_ROWS
+#define TBS_ROW2048_ROWS 2
+#define TBS_ROW2048_NT 256
+#define TBS_ROW2048_MINB 3
+#endif
+template <int R_, int NT_, int MB_> struct RowCfgT { static constexpr int ROWS = R_, NT = NT_, MINB = MB_; };
+template <> struct RowCfg<2048> : RowCfgT<TBS_ROW2048_ROWS, TBS_ROW2048_NT, TBS_ROW2048_MINB> {};
+template <> struct RowCfg<4096> { static constexpr int ROWS = 1, NT = 256, MINB = 3; };
 
 template <int N, int MODE>
 static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
@@ -58,7 +69,7 @@ template <int N, bool FIRST>
 static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
     constexpr size_t smem = 2 * (size_t)C::ROWS * RowLay<N>::PITCH * sizeof(float2);
-    auto kern = k_row<N, C::ROWS, C::NT, FIRST>;
+    auto kern = k_row<N, C::ROWS, C::NT, C::MINB, FIRST>;
     if (set_attr) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     kern<<<(unsigned)(a.rows / C::ROWS), C::NT, smem, st>>>(a);
     return cudaGetLastError();

@@ -38,8 +38,8 @@ template <> struct Radix<64>   { static constexpr int R1 = 8,  R2 = 0,  RL = 8; 
 template <> struct Radix<128>  { static constexpr int R1 = 16, R2 = 0,  RL = 8;  };
 template <> struct Radix<256>  { static constexpr int R1 = 16, R2 = 0,  RL = 16; };
 template <> struct Radix<512>  { static constexpr int R1 = 8,  R2 = 8,  RL = 8;  };
-template <> struct Radix<1024> { static constexpr int R1 = 16, R2 = 8,  RL = 8;  };
-template <> struct Radix<2048> { static constexpr int R1 = 16, R2 = 16, RL = 8;  };
+template <> struct Radix<1024> { static constexpr int R1 = 8,  R2 = 8,  RL = 16; };
+template <> struct Radix<2048> { static constexpr int R1 = 8,  R2 = 16, RL = 16; };
 template <> struct Radix<4096> { static constexpr int R1 = 16, R2 = 16, RL = 16; };
 
 __host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }

@@ -165,8 +165,8 @@ __device__ __forceinline__ void load_chunk(float2 (&v)[RL], const float2 *g) {
 
 // FIRST = true : forward half only, w = src * src_scale (term 0: u_0 = G S, Eq. 20)
 // FIRST = false: inverse half (K3) + forward half (K1) of the next term
-template <int N, int ROWS, int NT, bool FIRST>
-__global__ void __launch_bounds__(NT) k_row(RowArgs a) {
+template <int N, int ROWS, int NT, int MINB, bool FIRST>
+__global__ void __launch_bounds__(NT, MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
