@@ -21,7 +21,7 @@ template <int T_, int NT_> struct ColCfgT { static constexpr int T = T_, NT = NT
 template <> struct ColCfg<2048> : ColCfgT<TBS_COL2048_T, TBS_COL2048_NT> {};
 template <> struct ColCfg<4096> { static constexpr int T = 2,  NT = 512; };
 
-// Row kernels: ROWS rows per CTA, NT threads.  Shared memory = 2*ROWS*(N + N/16)*8 bytes.
+// Row kernels: ROWS rows per CTA, NT threads, at least MINB CTAs per SM (register cap).  Shared memory = 2*ROWS*(N + N/16)*8 bytes.
 template <int N> struct RowCfg;
 template <> struct RowCfg<32> { static constexpr int ROWS = 16, NT = 64, MINB = 4; };
 template <> struct RowCfg<64> { static constexpr int ROWS = 8, NT = 64, MINB = 4; };
@@ -32,11 +32,11 @@ template <> struct RowCfg<1024> { static constexpr int ROWS = 2, NT = 128, MINB 
 #ifndef TBS_ROW2048_ROWS
 #define TBS_ROW2048_ROWS 2
 #define TBS_ROW2048_NT 256
-#define TBS_ROW2048_MINB 3
+#define TBS_ROW2048_MINB 2
 #endif
 template <int R_, int NT_, int MB_> struct RowCfgT { static constexpr int ROWS = R_, NT = NT_, MINB = MB_; };
 template <> struct RowCfg<2048> : RowCfgT<TBS_ROW2048_ROWS, TBS_ROW2048_NT, TBS_ROW2048_MINB> {};
-template <> struct RowCfg<4096> { static constexpr int ROWS = 1, NT = 256, MINB = 3; };
+template <> struct RowCfg<4096> { static constexpr int ROWS = 1, NT = 256, MINB = 2; };
 
 template <int N, int MODE>
 static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
