@@ -4,49 +4,103 @@
 
 namespace tbs {
 
-// Column-tile kernels: T adjacent lines per CTA, NT threads.  Shared memory = 2*N*T*8 bytes
-// (both parity halves of the padded line).
+// Column-tile kernel k_col (3-D y passes, N <= 512): T adjacent lines per CTA, NT threads.  Shared memory = 2*N*T*8 bytes
+// (both parity halves of the padded line) + N*T*8 bytes of input staging (CONV, FWD).
 template <int N> struct ColCfg;
 template <> struct ColCfg<32>   { static constexpr int T = 16, NT = 64;  };
 template <> struct ColCfg<64>   { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<128>  { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<256>  { static constexpr int T = 16, NT = 256; };
 template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
-template <> struct ColCfg<1024> { static constexpr int T = 8,  NT = 512; };
-#ifndef TBS_COL2048_T
-#define TBS_COL2048_T 4
-#define TBS_COL2048_NT 512
-#endif
-template <int T_, int NT_> struct ColCfgT { static constexpr int T = T_, NT = NT_; };
-template <> struct ColCfg<2048> : ColCfgT<TBS_COL2048_T, TBS_COL2048_NT> {};
-template <> struct ColCfg<4096> { static constexpr int T = 2,  NT = 512; };
 
-// Row kernels: ROWS rows per CTA, NT threads, at least MINB CTAs per SM (register cap).  Shared memory = 2*ROWS*(N + N/16)*8 bytes.
-template <int N> struct RowCfg;
-template <> struct RowCfg<32> { static constexpr int ROWS = 16, NT = 64, MINB = 4; };
-template <> struct RowCfg<64> { static constexpr int ROWS = 8, NT = 64, MINB = 4; };
-template <> struct RowCfg<128> { static constexpr int ROWS = 8, NT = 64, MINB = 4; };
-template <> struct RowCfg<256> { static constexpr int ROWS = 4, NT = 64, MINB = 4; };
-template <> struct RowCfg<512> { static constexpr int ROWS = 2, NT = 128, MINB = 4; };
-template <> struct RowCfg<1024> { static constexpr int ROWS = 2, NT = 128, MINB = 3; };
-#ifndef TBS_ROW2048_ROWS
-#define TBS_ROW2048_ROWS 2
-#define TBS_ROW2048_NT 256
-#define TBS_ROW2048_MINB 2
+// Row kernel: GROUPS independent line groups per CTA (a group = N/16 threads on one row, or one warp
+// on 32/(N/16) rows), at least MINB CTAs per SM (register cap).  Shared memory per row =
+// 2*(N + N/16)*8 bytes of work area + N*16 bytes of W staging.
+template <int N> struct RowCfg { static constexpr int GROUPS = 4, MINB = 3; };   // N <= 512
+#ifndef TBS_ROW1024_GROUPS
+#define TBS_ROW1024_GROUPS 2
+#define TBS_ROW1024_MINB 3
 #endif
-template <int R_, int NT_, int MB_> struct RowCfgT { static constexpr int ROWS = R_, NT = NT_, MINB = MB_; };
-template <> struct RowCfg<2048> : RowCfgT<TBS_ROW2048_ROWS, TBS_ROW2048_NT, TBS_ROW2048_MINB> {};
-template <> struct RowCfg<4096> { static constexpr int ROWS = 1, NT = 256, MINB = 2; };
+#ifndef TBS_ROW2048_GROUPS
+#define TBS_ROW2048_GROUPS 1
+#define TBS_ROW2048_MINB 3
+#endif
+template <> struct RowCfg<1024> { static constexpr int GROUPS = TBS_ROW1024_GROUPS, MINB = TBS_ROW1024_MINB; };
+template <> struct RowCfg<2048> { static constexpr int GROUPS = TBS_ROW2048_GROUPS, MINB = TBS_ROW2048_MINB; };
+template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 1; };
+
+// Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads.  Shared memory =
+// 2*T*(N + N/16 + 4)*8 bytes of work area + N*T*8 bytes of input staging.
+template <int N> struct ConvCfg { static constexpr int T = 16, MINB = 2; };    // N <= 256
+template <> struct ConvCfg<512>  { static constexpr int T = 8, MINB = 2; };
+#ifndef TBS_CONV1024_T
+#define TBS_CONV1024_T 4
+#endif
+template <> struct ConvCfg<1024> { static constexpr int T = TBS_CONV1024_T, MINB = 2; };
+template <> struct ConvCfg<2048> { static constexpr int T = 4, MINB = 1; };
+template <> struct ConvCfg<4096> { static constexpr int T = 2, MINB = 1; };
+
+// Persistent grids: number of CTAs that are resident at once (SMs x CTAs per SM), found once per
+// kernel instance when the plan sets the shared-memory attribute.
+static inline int resident_ctas(const void *kern, int threads, size_t smem) {
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    return sms * per_sm;
+}
 
 template <int N, int MODE>
 static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
     using C = ColCfg<N>;
-    constexpr size_t smem = 2 * (size_t)N * C::T * sizeof(float2);
+    constexpr size_t smem = (size_t)N * C::T * sizeof(float2) * (MODE == MODE_INV ? 2 : 3);
     auto kern = k_col<N, C::T, C::NT, MODE>;
-    if (set_attr) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const unsigned grid = (unsigned)(n_outer * (a.inner_len / C::T));
-    kern<<<grid, C::NT, smem, st>>>(a);
+    static int cap = 0;
+    if (set_attr) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) cap = resident_ctas((const void *)kern, C::NT, smem);
+        return e;
+    }
+    ColArgs b = a;
+    b.n_outer = n_outer;
+    const long long total = (long long)n_outer * (a.inner_len / C::T);
+    const unsigned grid = (unsigned)(total < cap ? total : cap);
+    kern<<<grid, C::NT, smem, st>>>(b);
     return cudaGetLastError();
+}
+
+template <int N>
+static cudaError_t launch_conv_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
+    constexpr int T = ConvCfg<N>::T;
+    constexpr int NT = T * tpl_of(N);
+    constexpr size_t smem = (2 * (size_t)T * RowLay<N, conv_pad(N, T)>::PITCH + (size_t)N * T) * sizeof(float2);
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
+    static int cap = 0;
+    if (set_attr) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) cap = resident_ctas((const void *)kern, NT, smem);
+        return e;
+    }
+    ColArgs b = a;
+    b.n_outer = n_outer;
+    const long long total = (long long)n_outer * (a.inner_len / T);
+    kern<<<(unsigned)(total < cap ? total : cap), NT, smem, st>>>(b);
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_conv(int N, const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr = false) {
+    switch (N) {
+        case 32:   return launch_conv_t<32>(a, n_outer, st, set_attr);
+        case 64:   return launch_conv_t<64>(a, n_outer, st, set_attr);
+        case 128:  return launch_conv_t<128>(a, n_outer, st, set_attr);
+        case 256:  return launch_conv_t<256>(a, n_outer, st, set_attr);
+        case 512:  return launch_conv_t<512>(a, n_outer, st, set_attr);
+        case 1024: return launch_conv_t<1024>(a, n_outer, st, set_attr);
+        case 2048: return launch_conv_t<2048>(a, n_outer, st, set_attr);
+        case 4096: return launch_conv_t<4096>(a, n_outer, st, set_attr);
+        default: break;
+    }
+    return cudaErrorInvalidValue;
 }
 
 template <int MODE>
@@ -57,9 +111,6 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
         case 128:  return launch_col_t<128, MODE>(a, n_outer, st, set_attr);
         case 256:  return launch_col_t<256, MODE>(a, n_outer, st, set_attr);
         case 512:  return launch_col_t<512, MODE>(a, n_outer, st, set_attr);
-        case 1024: if (MODE == MODE_CONV) return launch_col_t<1024, MODE_CONV>(a, n_outer, st, set_attr); break;
-        case 2048: if (MODE == MODE_CONV) return launch_col_t<2048, MODE_CONV>(a, n_outer, st, set_attr); break;
-        case 4096: if (MODE == MODE_CONV) return launch_col_t<4096, MODE_CONV>(a, n_outer, st, set_attr); break;
         default: break;
     }
     return cudaErrorInvalidValue;
@@ -68,10 +119,21 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
 template <int N, bool FIRST>
 static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
-    constexpr size_t smem = 2 * (size_t)C::ROWS * RowLay<N>::PITCH * sizeof(float2);
-    auto kern = k_row<N, C::ROWS, C::NT, C::MINB, FIRST>;
-    if (set_attr) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    kern<<<(unsigned)(a.rows / C::ROWS), C::NT, smem, st>>>(a);
+    constexpr int TPL = tpl_of(N);
+    constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;
+    constexpr int NT = C::GROUPS * TPL * GR;
+    constexpr int ROWS = C::GROUPS * GR;
+    constexpr size_t smem = 2 * (size_t)ROWS * RowLay<N>::PITCH * sizeof(float2) +
+                            (FIRST ? 0 : (size_t)ROWS * N * sizeof(float4));
+    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST>;
+    static int cap = 0;
+    if (set_attr) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) cap = resident_ctas((const void *)kern, NT, smem);
+        return e;
+    }
+    const int tiles = (a.rows / GR + C::GROUPS - 1) / C::GROUPS;
+    kern<<<(unsigned)(tiles < cap ? tiles : cap), NT, smem, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -31,6 +31,38 @@ __device__ __forceinline__ float2 cmulc(float2 a, float2 b) {
     return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
 }
 
+// ---- asynchronous copies (global -> shared) -------------------------------------------------------
+// Row tiles are contiguous in global memory and come in with one bulk copy (TMA engine, completion
+// on an mbarrier); column tiles are N short segments and come in with 16-byte cp.async (LDGSTS).
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void cp_async16(void *dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ---- radix plan ------------------------------------------------------------------------------
 template <int N> struct Radix;
 template <> struct Radix<32>   { static constexpr int R1 = 8,  R2 = 0,  RL = 4;  };
@@ -89,26 +121,22 @@ __device__ __forceinline__ void bfly(float2 (&v)[R]) {
 
 // ---- per-stage twiddle look-up tables ---------------------------------------------------------
 // A stage with block length LB = R*S needs w_LB^(k t), k < R, for its sub-index t < S.  The tables
-// are stored [t][R] (float2) so that one thread fetches its R twiddles with R/2 128-bit loads from
-// one contiguous, 16-byte-aligned chunk (built in double by k_stage_lut, setup_kernels.cuh):
-//   lutA[t][k] = w_N^(k t)            first / last stage, even-frequency half (parity 0)
-//   lutB[t][k] = w_2N^((2k+1) t)      first / last stage, odd-frequency half  (parity 1): the
+// are stored k-major, [R][S] (float2), so that the threads of a warp -- consecutive t -- fetch each
+// twiddle with one contiguous 256-byte load (built in double by k_stage_lut, setup_kernels.cuh):
+//   lutA[k][t] = w_N^(k t)            first / last stage, even-frequency half (parity 0)
+//   lutB[k][t] = w_2N^((2k+1) t)      first / last stage, odd-frequency half  (parity 1): the
 //                                     zero-padding twist w_2N^(pos), pos = t + j*S1, factors into
 //                                     w_2N^t (folded into the table) and the constant w_(2 R1)^j
-//   lutC[t][k] = w_S1^(k t)           middle stage (three-stage plans only)
+//   lutC[k][t] = w_S1^(k t)           middle stage (three-stage plans only)
 struct Luts {
     const float2 *A, *B, *C;
 };
 
-template <int R>
+// K0 = 1 skips k = 0 (the twiddle is 1 in tables A and C).
+template <int R, int S, int K0>
 __device__ __forceinline__ void load_tw(float2 (&w)[R], const float2 *__restrict__ lut, int t) {
-    const float4 *p = reinterpret_cast<const float4 *>(lut + (size_t)t * R);
 #pragma unroll
-    for (int i = 0; i < R / 2; ++i) {
-        const float4 v = __ldg(p + i);
-        w[2 * i] = make_float2(v.x, v.y);
-        w[2 * i + 1] = make_float2(v.z, v.w);
-    }
+    for (int k = K0; k < R; ++k) w[k] = __ldg(lut + k * S + t);
 }
 
 // d * w_32^(idx) with sign SGN; idx in [0, 16).
@@ -152,59 +180,88 @@ struct ColLay {
     template <int NBL>
     __device__ static __forceinline__ void split(int w, int &line, int &b) { line = w % T_; b = w / T_; }
 };
-// Row tile: each line contiguous, one pad slot per 16 positions.
-template <int N>
+// Row tile: each line contiguous, one pad slot per 16 positions, PAD extra slots per line (PAD = 4
+// makes a cooperative read across 4 lines x 4 positions conflict-free for N >= 256).
+template <int N, int PAD = 0>
 struct RowLay {
-    static constexpr int PITCH = N + N / 16;
+    static constexpr int PITCH = N + N / 16 + PAD;
     __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + pos + (pos >> 4); }
     template <int NBL>
     __device__ static __forceinline__ void split(int w, int &line, int &b) { b = w % NBL; line = w / NBL; }
 };
+
+// Threads that own one line in the line-group kernels (k_row, k_conv): one radix-16 item each in
+// the widest stage.  Groups of TPL >= 32 threads synchronise on a named barrier of their own,
+// smaller groups share a warp and use __syncwarp, so no stage waits for the whole CTA.
+// Extra slots per line of the k_conv work area: the cooperative copy-out reads 2 chunks x 8 positions
+// (T = 4) or 4 chunks x 4 positions (T >= 8) per half-warp, conflict-free when the pitch is 4 resp.
+// 2 modulo 16.
+__host__ __device__ constexpr int conv_pad(int N, int T) {
+    return ((T >= 8 ? 2 : 4) + 32 - (N + N / 16) % 16) % 16;
+}
+__host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
+template <int GT>
+__device__ __forceinline__ void group_sync(int gid) {
+    if (GT <= 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(gid + 1), "n"(GT) : "memory");
+}
 
 // ---- in-place stages on shared memory, both parity halves at once --------------------------------
 // sm holds the even-frequency half at [0, HALF) and the odd-frequency half at [HALF, 2 HALF); one
 // work item is the pair of butterflies (parity 0, parity 1) at the same (line, block, t), which
 // share their twiddles.  Block length LB, radix R, sub-stride S = LB/R.
 // FWD (DIF): butterfly then twiddle w_LB^(k t);  inverse (DIT): conj twiddle then butterfly.
+template <int N, int LB, int R, bool FWD, class Lay, int HALF>
+__device__ __forceinline__ void stage_item(float2 *sm, const float2 *__restrict__ lut, int line, int b) {
+    constexpr int S = LB / R;
+    const int t = b % S;
+    const int base = (b / S) * LB + t;
+    float2 tw[R];
+    if (S > 1) load_tw<R, S, 1>(tw, lut, t);
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        float2 *s = sm + p * HALF;
+        float2 v[R];
+        if (FWD) {
+#pragma unroll
+            for (int j = 0; j < R; ++j) v[j] = s[Lay::addr(line, base + j * S)];
+            bfly<R, -1>(v);
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const int k = brev(i, R);
+                float2 o = v[i];
+                if (S > 1 && k > 0) o = cmul(o, tw[k]);
+                s[Lay::addr(line, base + k * S)] = o;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < R; ++k) {
+                float2 x = s[Lay::addr(line, base + k * S)];
+                if (S > 1 && k > 0) x = cmulc(x, tw[k]);
+                v[k] = x;
+            }
+            bfly<R, +1>(v);
+#pragma unroll
+            for (int i = 0; i < R; ++i) s[Lay::addr(line, base + brev(i, R) * S)] = v[i];
+        }
+    }
+}
+// all lines of a CTA tile, items dealt round-robin to the NT threads
 template <int N, int LB, int R, bool FWD, class Lay, int NT, int HALF>
 __device__ __forceinline__ void stage_pair(float2 *sm, const float2 *__restrict__ lut, int tid, int total) {
-    constexpr int S = LB / R;
     constexpr int NBL = N / R;
     for (int w = tid; w < total; w += NT) {
         int line, b;
         Lay::template split<NBL>(w, line, b);
-        const int t = b % S;
-        const int base = (b / S) * LB + t;
-        float2 tw[R];
-        if (S > 1) load_tw<R>(tw, lut, t);
-#pragma unroll
-        for (int p = 0; p < 2; ++p) {
-            float2 *s = sm + p * HALF;
-            float2 v[R];
-            if (FWD) {
-#pragma unroll
-                for (int j = 0; j < R; ++j) v[j] = s[Lay::addr(line, base + j * S)];
-                bfly<R, -1>(v);
-#pragma unroll
-                for (int i = 0; i < R; ++i) {
-                    const int k = brev(i, R);
-                    float2 o = v[i];
-                    if (S > 1 && k > 0) o = cmul(o, tw[k]);
-                    s[Lay::addr(line, base + k * S)] = o;
-                }
-            } else {
-#pragma unroll
-                for (int k = 0; k < R; ++k) {
-                    float2 x = s[Lay::addr(line, base + k * S)];
-                    if (S > 1 && k > 0) x = cmulc(x, tw[k]);
-                    v[k] = x;
-                }
-                bfly<R, +1>(v);
-#pragma unroll
-                for (int i = 0; i < R; ++i) s[Lay::addr(line, base + brev(i, R) * S)] = v[i];
-            }
-        }
+        stage_item<N, LB, R, FWD, Lay, HALF>(sm, lut, line, b);
     }
+}
+// one line, items dealt to the TPL threads that own it
+template <int N, int LB, int R, bool FWD, class Lay, int TPL, int HALF>
+__device__ __forceinline__ void stage_line(float2 *sm, const float2 *__restrict__ lut, int line, int lt) {
+    constexpr int NBL = N / R;
+#pragma unroll 1
+    for (int b = lt; b < NBL; b += TPL) stage_item<N, LB, R, FWD, Lay, HALF>(sm, lut, line, b);
 }
 
 // First forward stage from registers: x[j] is the input at position t + j*S1 (natural order).
@@ -215,7 +272,7 @@ __device__ __forceinline__ void first_fwd_pair(const float2 (&x)[R1], int line, 
     constexpr int S1 = N / R1;
     float2 tw[R1];
     float2 v[R1];
-    load_tw<R1>(tw, L.A, t);
+    load_tw<R1, S1, 1>(tw, L.A, t);
 #pragma unroll
     for (int j = 0; j < R1; ++j) v[j] = x[j];
     bfly<R1, -1>(v);
@@ -224,7 +281,7 @@ __device__ __forceinline__ void first_fwd_pair(const float2 (&x)[R1], int line, 
         const int k = brev(i, R1);
         sm[Lay::addr(line, t + k * S1)] = k > 0 ? cmul(v[i], tw[k]) : v[i];
     }
-    load_tw<R1>(tw, L.B, t);
+    load_tw<R1, S1, 0>(tw, L.B, t);
 #pragma unroll
     for (int j = 0; j < R1; ++j) v[j] = x[j];
     twist_const<R1, -1>(v);
@@ -244,14 +301,14 @@ __device__ __forceinline__ void last_inv_pair(float2 (&z)[R1], int line, int t, 
     constexpr int S1 = N / R1;
     float2 tw[R1];
     float2 v[R1], u[R1];
-    load_tw<R1>(tw, L.A, t);
+    load_tw<R1, S1, 1>(tw, L.A, t);
 #pragma unroll
     for (int k = 0; k < R1; ++k) {
         const float2 a = sm[Lay::addr(line, t + k * S1)];
         v[k] = k > 0 ? cmulc(a, tw[k]) : a;
     }
     bfly<R1, +1>(v);
-    load_tw<R1>(tw, L.B, t);
+    load_tw<R1, S1, 0>(tw, L.B, t);
 #pragma unroll
     for (int k = 0; k < R1; ++k) u[k] = cmulc(sm[HALF + Lay::addr(line, t + k * S1)], tw[k]);
     bfly<R1, +1>(u);
@@ -262,54 +319,56 @@ __device__ __forceinline__ void last_inv_pair(float2 (&z)[R1], int line, int t, 
     }
 }
 
-// 1/d to ~1 ulp without the IEEE-division slow path: MUFU.RCP + one Newton step.  d >= e^2 > 0.
-__device__ __forceinline__ float rcp_nr(float d) {
+// 1/d by MUFU.RCP (rcp.approx: relative error <= 2^-23), without the IEEE-division slow path.
+__device__ __forceinline__ float rcp_fast(float d) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d));
-    return fmaf(r, fmaf(-d, r, 1.0f), r);
+    return r;
 }
 
 // Fused middle of the convolution: last forward stage (contiguous blocks of RL), multiply by
 // ghat, first inverse stage -- all in registers (north_star: "pointwise G multiply fused into the
 // last forward and first inverse butterfly stage").
-//   ghat' = scale / (a - i e),  a = a_line + p2[P],  e = eps/k0^2   (non-dimensional)
+//   k0^2 ghat = 1/(a - i e) = (a + i e)/(a^2 + e^2),  a = a_line + p2[P],  e = eps/k0^2
+// (non-dimensional; the 1/prod(2N) of the inverse transforms is applied by k_row).
+template <int N, int RL, class Lay, int HALF>
+__device__ __forceinline__ void mid_conv_item(float2 *sm, int line, int b, const float *__restrict__ p2line,
+                                              float a_line, float e) {
+    const int base = b * RL;
+    const float e2 = e * e;
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        float2 *s = sm + p * HALF;
+        float2 v[RL];
+        float pp[RL];
+        // table in the transposed order [half][j][block]: consecutive threads, consecutive words
+#pragma unroll
+        for (int j = 0; j < RL; ++j) pp[j] = __ldg(p2line + p * N + j * (N / RL) + b);
+#pragma unroll
+        for (int j = 0; j < RL; ++j) v[j] = s[Lay::addr(line, base + j)];
+        bfly<RL, -1>(v);
+        float2 u[RL];
+#pragma unroll
+        for (int i = 0; i < RL; ++i) {
+            const int k = brev(i, RL);
+            const float a = a_line + pp[k];
+            const float r = rcp_fast(fmaf(a, a, e2));
+            const float tx = v[i].x * r, ty = v[i].y * r;
+            u[k] = make_float2(fmaf(tx, a, -ty * e), fmaf(tx, e, ty * a));
+        }
+        bfly<RL, +1>(u);
+#pragma unroll
+        for (int i = 0; i < RL; ++i) s[Lay::addr(line, base + brev(i, RL))] = u[i];
+    }
+}
 template <int N, int RL, class Lay, int NT, int HALF>
 __device__ __forceinline__ void mid_conv_pair(float2 *sm, int tid, int total, const float *__restrict__ p2line,
-                                              float a_line, float e, float scale) {
+                                              float a_line, float e) {
     constexpr int NBL = N / RL;
-    const float e2 = e * e;
     for (int w = tid; w < total; w += NT) {
         int line, b;
         Lay::template split<NBL>(w, line, b);
-        const int base = b * RL;
-#pragma unroll
-        for (int p = 0; p < 2; ++p) {
-            float2 *s = sm + p * HALF;
-            float2 v[RL];
-            float pp[RL];
-            // RL consecutive table entries, 16-byte aligned
-            const float4 *pt = reinterpret_cast<const float4 *>(p2line + p * N + base);
-#pragma unroll
-            for (int q = 0; q < RL / 4; ++q) {
-                const float4 f = __ldg(pt + q);
-                pp[4 * q] = f.x; pp[4 * q + 1] = f.y; pp[4 * q + 2] = f.z; pp[4 * q + 3] = f.w;
-            }
-#pragma unroll
-            for (int j = 0; j < RL; ++j) v[j] = s[Lay::addr(line, base + j)];
-            bfly<RL, -1>(v);
-            float2 u[RL];
-#pragma unroll
-            for (int i = 0; i < RL; ++i) {
-                const int k = brev(i, RL);
-                const float a = a_line + pp[k];
-                const float r = scale * rcp_nr(fmaf(a, a, e2));
-                const float gr = a * r, gi = e * r;
-                u[k] = make_float2(v[i].x * gr - v[i].y * gi, v[i].x * gi + v[i].y * gr);
-            }
-            bfly<RL, +1>(u);
-#pragma unroll
-            for (int i = 0; i < RL; ++i) s[Lay::addr(line, base + brev(i, RL))] = u[i];
-        }
+        mid_conv_item<N, RL, Lay, HALF>(sm, line, b, p2line, a_line, e);
     }
 }
 

@@ -27,7 +27,7 @@ struct Ctl {
     int n_terms;     // index of the last term added
 };
 
-enum { MODE_CONV = 0, MODE_FWD = 1, MODE_INV = 2 };
+enum { MODE_FWD = 1, MODE_INV = 2 };
 
 struct ColArgs {
     const float2 *in;
@@ -35,14 +35,18 @@ struct ColArgs {
     long long in_line_stride, out_line_stride;    // between consecutive positions of a line
     long long in_outer_stride, out_outer_stride;  // between consecutive outer indices
     int inner_len;                                // number of adjacent lines (multiple of T)
+    int n_outer;                                  // number of outer indices
     const float *p2_line;   // [2N] |p|^2/k0^2 of this axis, position order       (CONV)
     const float *p2_inner;  // [inner_len] of the inner (x) axis, position order  (CONV)
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
-    float e, scale;         // eps/k0^2 and 1/prod(2N)                            (CONV)
+    float e;                // eps/k0^2                                           (CONV)
     Luts lut;
     const Ctl *ctl;
 };
 
+// Persistent: each CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...  For CONV and FWD the N
+// input positions of the next tile are fetched with cp.async into a staging buffer while the
+// current tile computes.
 template <int N, int T, int NT, int MODE>
 __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     using P = Radix<N>;
@@ -50,86 +54,104 @@ __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
     static_assert((S1 * T) % NT == 0 && NT % T == 0, "tile/thread mismatch");
+    static_assert(T % 2 == 0, "16-byte staging copies need an even tile width");
     constexpr int NB = (S1 * T) / NT;  // first/last-stage butterfly pairs per thread
     constexpr int TSTEP = NT / T;
     constexpr int HALF = N * T;
     using Lay = ColLay<N, T, RL>;
-    extern __shared__ float2 sm[];
+    extern __shared__ __align__(128) float2 sm[];
+    float2 *stg = sm + 2 * HALF;  // [N][T] staged input tile (CONV, FWD)
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
     const int line = tid % T, t0 = tid / T;
     const int tiles = a.inner_len / T;
-    const int inner0 = (blockIdx.x % tiles) * T;
-    const int outer = blockIdx.x / tiles;
-    const float2 *in = a.in + (long long)outer * a.in_outer_stride + inner0 + line;
-    float2 *out = a.out + (long long)outer * a.out_outer_stride + inner0 + line;
+    const int total = tiles * a.n_outer;
 
-    // ---- forward: N inputs -> both halves in smem ----
-    if (MODE != MODE_INV) {
+    auto stage_tile = [&](int tile) {
+        const int inner0 = (tile % tiles) * T;
+        const int outer = tile / tiles;
+        const float2 *src = a.in + (long long)outer * a.in_outer_stride + inner0;
+        constexpr int CPR = T / 2;  // 16-byte chunks per position
+        for (int c = tid; c < N * CPR; c += NT) {
+            const int r = c / CPR, cc = c % CPR;
+            cp_async16(stg + r * T + 2 * cc, src + (long long)r * a.in_line_stride + 2 * cc);
+        }
+        cp_async_commit();
+    };
+    if (MODE != MODE_INV && (int)blockIdx.x < total) stage_tile(blockIdx.x);
+
+    for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+        const int inner0 = (tile % tiles) * T;
+        const int outer = tile / tiles;
+        const float2 *in = a.in + (long long)outer * a.in_outer_stride + inner0 + line;
+        float2 *out = a.out + (long long)outer * a.out_outer_stride + inner0 + line;
+
+        // ---- forward: N inputs -> both halves in smem ----
+        if (MODE != MODE_INV) {
+            cp_async_wait_all();
+            __syncthreads();  // staged tile visible; previous tile's readers of the work area are done
+#pragma unroll
+            for (int i = 0; i < NB; ++i) {
+                const int t = t0 + i * TSTEP;
+                float2 x[R1];
+#pragma unroll
+                for (int j = 0; j < R1; ++j) x[j] = stg[(t + j * S1) * T + line];
+                first_fwd_pair<N, R1, Lay, HALF>(x, line, t, sm, a.lut);
+            }
+            __syncthreads();
+            if (tile + (int)gridDim.x < total) stage_tile(tile + gridDim.x);
+            if (R2 > 0) {
+                stage_pair<N, S1, R2s, true, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
+                __syncthreads();
+            }
+        }
+        if (MODE == MODE_FWD) {
+            // last forward stage straight to global: positions s*N + b*RL + k
+            for (int w = tid; w < (N / RL) * T; w += NT) {
+                const int b = w / T;
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    float2 v[RL];
+#pragma unroll
+                    for (int j = 0; j < RL; ++j) v[j] = sm[s * HALF + Lay::addr(line, b * RL + j)];
+                    bfly<RL, -1>(v);
+#pragma unroll
+                    for (int i = 0; i < RL; ++i)
+                        out[(long long)(s * N + b * RL + brev(i, RL)) * a.out_line_stride] = v[i];
+                }
+            }
+            continue;
+        } else {
+            // INV: first inverse stage straight from global
+            __syncthreads();  // previous tile's readers of the work area are done
+            for (int w = tid; w < (N / RL) * T; w += NT) {
+                const int b = w / T;
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    float2 v[RL];
+#pragma unroll
+                    for (int k = 0; k < RL; ++k) v[k] = in[(long long)(s * N + b * RL + k) * a.in_line_stride];
+                    bfly<RL, +1>(v);
+#pragma unroll
+                    for (int i = 0; i < RL; ++i) sm[s * HALF + Lay::addr(line, b * RL + brev(i, RL))] = v[i];
+                }
+            }
+            __syncthreads();
+        }
+        // ---- inverse: both halves -> N outputs ----
+        if (R2 > 0) {
+            stage_pair<N, S1, R2s, false, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
+            __syncthreads();
+        }
 #pragma unroll
         for (int i = 0; i < NB; ++i) {
             const int t = t0 + i * TSTEP;
-            float2 x[R1];
+            float2 z[R1];
+            last_inv_pair<N, R1, Lay, HALF>(z, line, t, sm, a.lut);
 #pragma unroll
-            for (int j = 0; j < R1; ++j) x[j] = in[(long long)(t + j * S1) * a.in_line_stride];
-            first_fwd_pair<N, R1, Lay, HALF>(x, line, t, sm, a.lut);
+            for (int j = 0; j < R1; ++j) out[(long long)(t + j * S1) * a.out_line_stride] = z[j];
         }
-        __syncthreads();
-        if (R2 > 0) {
-            stage_pair<N, S1, R2s, true, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
-            __syncthreads();
-        }
-    }
-    if (MODE == MODE_CONV) {
-        float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
-        if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
-        mid_conv_pair<N, RL, Lay, NT, HALF>(sm, tid, (N / RL) * T, a.p2_line, a_line, a.e, a.scale);
-        __syncthreads();
-    } else if (MODE == MODE_FWD) {
-        // last forward stage straight to global: positions s*N + b*RL + k
-        for (int w = tid; w < (N / RL) * T; w += NT) {
-            const int b = w / T;
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                float2 v[RL];
-#pragma unroll
-                for (int j = 0; j < RL; ++j) v[j] = sm[s * HALF + Lay::addr(line, b * RL + j)];
-                bfly<RL, -1>(v);
-#pragma unroll
-                for (int i = 0; i < RL; ++i)
-                    out[(long long)(s * N + b * RL + brev(i, RL)) * a.out_line_stride] = v[i];
-            }
-        }
-        return;
-    } else {
-        // INV: first inverse stage straight from global
-        for (int w = tid; w < (N / RL) * T; w += NT) {
-            const int b = w / T;
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                float2 v[RL];
-#pragma unroll
-                for (int k = 0; k < RL; ++k) v[k] = in[(long long)(s * N + b * RL + k) * a.in_line_stride];
-                bfly<RL, +1>(v);
-#pragma unroll
-                for (int i = 0; i < RL; ++i) sm[s * HALF + Lay::addr(line, b * RL + brev(i, RL))] = v[i];
-            }
-        }
-        __syncthreads();
-    }
-    // ---- inverse: both halves -> N outputs ----
-    if (R2 > 0) {
-        stage_pair<N, S1, R2s, false, Lay, NT, HALF>(sm, a.lut.C, tid, (N / R2s) * T);
-        __syncthreads();
-    }
-#pragma unroll
-    for (int i = 0; i < NB; ++i) {
-        const int t = t0 + i * TSTEP;
-        float2 z[R1];
-        last_inv_pair<N, R1, Lay, HALF>(z, line, t, sm, a.lut);
-#pragma unroll
-        for (int j = 0; j < R1; ++j) out[(long long)(t + j * S1) * a.out_line_stride] = z[j];
     }
 }
 
@@ -144,6 +166,7 @@ struct RowArgs {
     int ny;               // rows = ny * nz; row = z*ny + y
     int rows;
     float src_scale;      // FIRST: 1/k0^2
+    float scale;          // 1/prod(2 n): normalisation of the inverse transforms of all axes
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
@@ -151,84 +174,166 @@ struct RowArgs {
     Luts lut;
 };
 
-// RL contiguous complex values <-> registers with 128-bit accesses (RL*8 bytes, 16-byte aligned).
-template <int RL>
-__device__ __forceinline__ void load_chunk(float2 (&v)[RL], const float2 *g) {
-    const float4 *p = reinterpret_cast<const float4 *>(g);
-#pragma unroll
-    for (int q = 0; q < RL / 2; ++q) {
-        const float4 f = p[q];
-        v[2 * q] = make_float2(f.x, f.y);
-        v[2 * q + 1] = make_float2(f.z, f.w);
-    }
-}
+// ---------------------------------------------------------------------------------------------------
+// Line-group kernels.  A line (a grid row for k_row, a column for k_conv) is owned by TPL = N/16
+// threads for the whole of its transform; those threads synchronise among themselves only (named
+// barrier, or __syncwarp when several lines share a warp), so the shared-memory traffic of one
+// group overlaps the butterflies of another instead of every stage waiting for the whole CTA.
+// ---------------------------------------------------------------------------------------------------
 
+// Layout of a W row along x (2N complex values): the parity halves are interleaved and the last
+// digit is transposed, so that every access of k_row is a 16-byte-per-lane, lane-contiguous one:
+//   column c = 2 q + s,  q = k * (N/RL) + b   <->   half s, position pos = b * RL + k
+// (b = block of the contiguous last forward / first inverse stage, k = index inside the block).
+// The x axis table of the Green's spectrum is built in this column order (k_axis_table).
+//
 // FIRST = true : forward half only, w = src * src_scale (term 0: u_0 = G S, Eq. 20)
 // FIRST = false: inverse half (K3) + forward half (K1) of the next term
-template <int N, int ROWS, int NT, int MINB, bool FIRST>
-__global__ void __launch_bounds__(NT, MINB) k_row(RowArgs a) {
+// Persistent and group-independent: group G of CTA B walks row tiles (B*GROUPS + G) + i*gridDim.x*
+// GROUPS; the W rows of its next tile arrive by one bulk copy (completion on the group's mbarrier)
+// in a staging buffer while the current tile computes.
+template <int N, int GROUPS, int MINB, bool FIRST>
+__global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
-    static_assert((ROWS * S1) % NT == 0, "tile/thread mismatch");
-    constexpr int NB = (ROWS * S1) / NT;
+    constexpr int NBL = N / RL;
     constexpr int M = 2 * N;
+    constexpr int TPL = tpl_of(N);
+    constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;  // rows per group
+    constexpr int GT = TPL * GR;                   // threads per group
+    constexpr int NT = GROUPS * GT;
+    constexpr int ROWS = GROUPS * GR;
     using Lay = RowLay<N>;
     constexpr int HALF = ROWS * Lay::PITCH;
-    extern __shared__ float2 sm[];
+    extern __shared__ __align__(128) float2 sm[];
+    float4 *stg = reinterpret_cast<float4 *>(sm + 2 * HALF);  // [ROWS][N] staged W rows
     __shared__ float red[2][32];
+    __shared__ __align__(8) uint64_t mbar[GROUPS];
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
-    const int row0 = blockIdx.x * ROWS;
-    float2 x[NB][R1];
+    const int g = tid / GT, gl = tid % GT;
+    const int l = g * GR + gl / TPL;  // CTA-local line
+    const int lt = gl % TPL;
+    const int ngt = a.rows / GR;      // group tiles
+    const int gstride = gridDim.x * GROUPS;
     const int term = FIRST ? 0 : a.ctl->term;
+    constexpr uint32_t TILE_BYTES = (uint32_t)GR * M * sizeof(float2);
+    uint32_t phase = 0;
+    float uu = 0.f, pp = 0.f;
+    int gt = blockIdx.x * GROUPS + g;
+    if (!FIRST) {
+        if (tid == 0)
+            for (int i = 0; i < GROUPS; ++i) mbar_init(&mbar[i], 1);
+        __syncthreads();
+        if (gl == 0 && gt < ngt) {
+            mbar_expect_tx(&mbar[g], TILE_BYTES);
+            bulk_g2s(stg + g * GR * N, a.W + (long long)gt * GR * M, TILE_BYTES, &mbar[g]);
+        }
+    }
+
+#pragma unroll 1
+    for (; gt < ngt; gt += gstride) {
+        const int row = gt * GR + gl / TPL;
+        float wrow = a.scale;
+        if (!FIRST) {
+            // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
+            // pull the p and V rows of this tile towards L2 while the W rows arrive
+            for (int i = gl; i < GR * N / 16; i += GT) {
+                prefetch_l2(a.p + (long long)gt * GR * N + i * 16);
+                prefetch_l2(a.V + (long long)gt * GR * N + i * 16);
+            }
+            wrow *= __ldg(&a.ay[row % a.ny]);
+            if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
+            mbar_wait(&mbar[g], phase);
+            phase ^= 1u;
+            // first inverse stage (contiguous blocks of RL) from the staged rows
+#pragma unroll 1
+            for (int b = lt; b < NBL; b += TPL) {
+                float2 v0[RL], v1[RL];
+#pragma unroll
+                for (int k = 0; k < RL; ++k) {
+                    const float4 f = stg[l * N + k * NBL + b];
+                    v0[k] = make_float2(f.x, f.y);
+                    v1[k] = make_float2(f.z, f.w);
+                }
+                bfly<RL, +1>(v0);
+#pragma unroll
+                for (int i = 0; i < RL; ++i) sm[Lay::addr(l, b * RL + brev(i, RL))] = v0[i];
+                bfly<RL, +1>(v1);
+#pragma unroll
+                for (int i = 0; i < RL; ++i) sm[HALF + Lay::addr(l, b * RL + brev(i, RL))] = v1[i];
+            }
+            group_sync<GT>(g);
+            // the group's staging rows are free: fetch the W rows of its next tile
+            if (gl == 0 && gt + gstride < ngt) {
+                mbar_expect_tx(&mbar[g], TILE_BYTES);
+                bulk_g2s(stg + g * GR * N, a.W + (long long)(gt + gstride) * GR * M, TILE_BYTES, &mbar[g]);
+            }
+            if (R2 > 0) {
+                stage_line<N, S1, R2s, false, Lay, TPL, HALF>(sm, a.lut.C, l, lt);
+                group_sync<GT>(g);
+            }
+        }
+        // last inverse stage + crop + window + accumulate + V.u + first forward stage; a thread
+        // writes the slots it has just read, so the items need no barrier between them
+#pragma unroll 1
+        for (int t = lt; t < S1; t += TPL) {
+            float2 x[R1];
+            if (!FIRST) {
+                last_inv_pair<N, R1, Lay, HALF>(x, l, t, sm, a.lut);
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const int pos = t + j * S1;
+                    const long long gi = (long long)row * N + pos;
+                    const float wgt = wrow * __ldg(&a.ax[pos]);
+                    float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
+                    float2 pv = u;
+                    if (term > 0) pv = cadd(a.p[gi], u);
+                    a.p[gi] = pv;
+                    uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
+                    pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
+                    x[j] = cmul(__ldg(&a.V[gi]), u);
+                }
+                if (!a.do_fwd) continue;
+            } else {
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const float2 v = a.src[(long long)row * N + t + j * S1];
+                    x[j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
+                }
+            }
+            first_fwd_pair<N, R1, Lay, HALF>(x, l, t, sm, a.lut);
+        }
+        group_sync<GT>(g);
+        if (!FIRST && !a.do_fwd) continue;
+        // ---------------- forward half: the remaining stages of FFT_x ----------------
+        if (R2 > 0) {
+            stage_line<N, S1, R2s, true, Lay, TPL, HALF>(sm, a.lut.C, l, lt);
+            group_sync<GT>(g);
+        }
+        // last forward stage (contiguous blocks of RL) straight to global memory.  A thread reads
+        // exactly the slots it writes in the first inverse stage of its next tile.
+#pragma unroll 1
+        for (int b = lt; b < NBL; b += TPL) {
+            float2 v0[RL], v1[RL];
+#pragma unroll
+            for (int j = 0; j < RL; ++j) v0[j] = sm[Lay::addr(l, b * RL + j)];
+            bfly<RL, -1>(v0);
+#pragma unroll
+            for (int j = 0; j < RL; ++j) v1[j] = sm[HALF + Lay::addr(l, b * RL + j)];
+            bfly<RL, -1>(v1);
+            float4 *gp = reinterpret_cast<float4 *>(a.W + (long long)row * M) + b;
+#pragma unroll
+            for (int i = 0; i < RL; ++i)
+                gp[brev(i, RL) * NBL] = make_float4(v0[i].x, v0[i].y, v1[i].x, v1[i].y);
+        }
+        if (FIRST) group_sync<GT>(g);  // the next tile's first stage writes slots other threads still read
+    }
 
     if (!FIRST) {
-        // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
-        // first inverse stage (contiguous blocks of RL) straight from global memory
-        for (int w = tid; w < ROWS * (N / RL); w += NT) {
-            const int b = w % (N / RL), l = w / (N / RL);
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                float2 v[RL];
-                load_chunk<RL>(v, a.W + (long long)(row0 + l) * M + s * N + b * RL);
-                bfly<RL, +1>(v);
-#pragma unroll
-                for (int i = 0; i < RL; ++i) sm[s * HALF + Lay::addr(l, b * RL + brev(i, RL))] = v[i];
-            }
-        }
-        __syncthreads();
-        if (R2 > 0) {
-            stage_pair<N, S1, R2s, false, Lay, NT, HALF>(sm, a.lut.C, tid, ROWS * (N / R2s));
-            __syncthreads();
-        }
-        // last inverse stage + crop + window + accumulate; the same thread later writes the same
-        // smem slots in the forward half, so no barrier is needed in between
-        float uu = 0.f, pp = 0.f;
-#pragma unroll
-        for (int i = 0; i < NB; ++i) {
-            const int w = tid + i * NT;
-            const int t = w % S1, l = w / S1;
-            last_inv_pair<N, R1, Lay, HALF>(x[i], l, t, sm, a.lut);
-            const int row = row0 + l;
-            float wrow = __ldg(&a.ay[row % a.ny]);
-            if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
-#pragma unroll
-            for (int j = 0; j < R1; ++j) {
-                const int pos = t + j * S1;
-                const long long gi = (long long)row * N + pos;
-                const float wgt = wrow * __ldg(&a.ax[pos]);
-                float2 u = make_float2(x[i][j].x * wgt, x[i][j].y * wgt);
-                float2 pv = u;
-                if (term > 0) pv = cadd(a.p[gi], u);
-                a.p[gi] = pv;
-                uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
-                pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
-                x[i][j] = cmul(__ldg(&a.V[gi]), u);
-            }
-        }
         // block reduction (warp shuffles, then one double atomic per CTA and quantity)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -263,48 +368,104 @@ __global__ void __launch_bounds__(NT, MINB) k_row(RowArgs a) {
                 }
             }
         }
-        if (!a.do_fwd) return;
-    } else {
-#pragma unroll
-        for (int i = 0; i < NB; ++i) {
-            const int w = tid + i * NT;
-            const int t = w % S1, l = w / S1;
+    }
+}
+
+// K2 (2-D) / the z pass (3-D): for each of T adjacent lines along a strided axis: pad, FFT, .ghat,
+// IFFT, crop, in place in global memory.  Persistent; tile i+1 is fetched with
+// cp.async into a staging buffer while tile i computes; the result goes back through the work area
+// so that global reads and writes are 16 bytes per lane over adjacent lines.  Between the three
+// CTA-wide barriers of a tile the T line groups run on their own barriers.
+template <int N, int T, int MINB>
+__global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
+    using P = Radix<N>;
+    constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
+    constexpr int R2s = R2 > 0 ? R2 : 2;
+    constexpr int S1 = N / R1;
+    constexpr int TPL = tpl_of(N);
+    constexpr int NT = T * TPL;
+    constexpr int GT = TPL >= 32 ? TPL : 32;
+    static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
+    constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
+    using Lay = RowLay<N, conv_pad(N, T)>;
+    constexpr int HALF = T * Lay::PITCH;
+    extern __shared__ __align__(128) float2 sm[];
+    // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
+    // 2c+1), the chunk index XOR-swizzled with the position so that the cp.async writes of a warp are
+    // contiguous and the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
+    float4 *stg = reinterpret_cast<float4 *>(sm + 2 * HALF);
+    if (a.ctl->done) return;
+
+    const int tid = threadIdx.x;
+    const int line = tid / TPL, lt = tid % TPL;
+    const int g = tid / GT;
+    const int tiles = a.inner_len / T;
+    const int total = tiles * a.n_outer;
+    auto swz = [](int r) { return CPR > 1 ? (r / (CPR >= 8 ? 1 : 8 / CPR)) % CPR : 0; };
+
+    auto stage_tile = [&](int tile) {
+        const float2 *src = a.in + (long long)(tile / tiles) * a.in_outer_stride + (tile % tiles) * T;
+#pragma unroll 4
+        for (int c = tid; c < N * CPR; c += NT) {
+            const int r = c / CPR, cc = c % CPR;
+            cp_async16(stg + r * CPR + (cc ^ swz(r)), src + (long long)r * a.in_line_stride + 2 * cc);
+        }
+        cp_async_commit();
+    };
+    if ((int)blockIdx.x < total) stage_tile(blockIdx.x);
+    const float2 *stg2 = reinterpret_cast<const float2 *>(stg) + (line & 1);
+
+#pragma unroll 1
+    for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+        const int inner0 = (tile % tiles) * T;
+        const int outer = tile / tiles;
+        cp_async_wait_all();
+        __syncthreads();  // staged tile visible; the copy-out of the previous tile has left the work area
+        // ---- forward: N inputs -> both halves ----
+#pragma unroll 1
+        for (int t = lt; t < S1; t += TPL) {
+            float2 x[R1];
 #pragma unroll
             for (int j = 0; j < R1; ++j) {
-                float2 v = a.src[(long long)(row0 + l) * N + t + j * S1];
-                x[i][j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
+                const int r = t + j * S1;
+                x[j] = stg2[2 * (r * CPR + ((line >> 1) ^ swz(r)))];
             }
+            first_fwd_pair<N, R1, Lay, HALF>(x, line, t, sm, a.lut);
         }
-    }
-
-    // ---------------- forward half: zero-pad (two parity halves), FFT_x ----------------
+        __syncthreads();  // staging buffer free (and the line groups are in step)
+        if (tile + (int)gridDim.x < total) stage_tile(tile + gridDim.x);
+        if (R2 > 0) {
+            stage_line<N, S1, R2s, true, Lay, TPL, HALF>(sm, a.lut.C, line, lt);
+            group_sync<GT>(g);
+        }
+        {
+            float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
+            if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
+#pragma unroll 1
+            for (int b = lt; b < N / RL; b += TPL) mid_conv_item<N, RL, Lay, HALF>(sm, line, b, a.p2_line, a_line, a.e);
+            group_sync<GT>(g);
+        }
+        // ---- inverse: both halves -> N outputs, left in the even half of the work area ----
+        if (R2 > 0) {
+            stage_line<N, S1, R2s, false, Lay, TPL, HALF>(sm, a.lut.C, line, lt);
+            group_sync<GT>(g);
+        }
+#pragma unroll 1
+        for (int t = lt; t < S1; t += TPL) {
+            float2 z[R1];
+            last_inv_pair<N, R1, Lay, HALF>(z, line, t, sm, a.lut);
 #pragma unroll
-    for (int i = 0; i < NB; ++i) {
-        const int w = tid + i * NT;
-        const int t = w % S1, l = w / S1;
-        first_fwd_pair<N, R1, Lay, HALF>(x[i], l, t, sm, a.lut);
-    }
-    __syncthreads();
-    if (R2 > 0) {
-        stage_pair<N, S1, R2s, true, Lay, NT, HALF>(sm, a.lut.C, tid, ROWS * (N / R2s));
+            for (int j = 0; j < R1; ++j) sm[Lay::addr(line, t + j * S1)] = z[j];
+        }
         __syncthreads();
-    }
-    // last forward stage (contiguous blocks of RL) straight to global memory
-    for (int w = tid; w < ROWS * (N / RL); w += NT) {
-        const int b = w % (N / RL), l = w / (N / RL);
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            float2 v[RL];
-#pragma unroll
-            for (int j = 0; j < RL; ++j) v[j] = sm[s * HALF + Lay::addr(l, b * RL + j)];
-            bfly<RL, -1>(v);
-            // v[i] = X[brev(i)]: gather into natural order and store 2 values per 128-bit write
-            float2 o[RL];
-#pragma unroll
-            for (int i = 0; i < RL; ++i) o[brev(i, RL)] = v[i];
-            float4 *g = reinterpret_cast<float4 *>(a.W + (long long)(row0 + l) * M + s * N + b * RL);
-#pragma unroll
-            for (int q = 0; q < RL / 2; ++q) g[q] = make_float4(o[2 * q].x, o[2 * q].y, o[2 * q + 1].x, o[2 * q + 1].y);
+        float2 *dst = a.out + (long long)outer * a.out_outer_stride + inner0;
+        // lanes: 4 (or CPR) adjacent chunks x 8 positions, conflict-free with the line pitch of conv_pad
+        constexpr int CL = CPR < 4 ? CPR : 4;
+#pragma unroll 4
+        for (int c = tid; c < N * CPR; c += NT) {
+            const int r = (c / CL) % N, cc = (c / (CL * N)) * CL + c % CL;
+            const float2 v0 = sm[Lay::addr(2 * cc, r)], v1 = sm[Lay::addr(2 * cc + 1, r)];
+            *reinterpret_cast<float4 *>(dst + (long long)r * a.out_line_stride + 2 * cc) = make_float4(v0.x, v0.y, v1.x, v1.y);
         }
     }
 }

@@ -5,15 +5,15 @@
 
 namespace tbs {
 
-// Per-stage twiddle tables (fft_engine.cuh "Luts"), evaluated in double:
-//   which = 0: lut[t][k] = exp(-2 pi i k t / L)            (L = N: table A;  L = S1: table C)
-//   which = 1: lut[t][k] = exp(-2 pi i (2k+1) t / (2 L))   (L = N: table B)
+// Per-stage twiddle tables (fft_engine.cuh "Luts"), k-major [R][S], evaluated in double:
+//   which = 0: lut[k][t] = exp(-2 pi i k t / L)            (L = N: table A;  L = S1: table C)
+//   which = 1: lut[k][t] = exp(-2 pi i (2k+1) t / (2 L))   (L = N: table B)
 // t < S = L / R, k < R.
 __global__ void k_stage_lut(float2 *lut, int L, int R, int which) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int S = L / R;
     if (i >= S * R) return;
-    const int t = i / R, k = i % R;
+    const int k = i / S, t = i % S;
     double s, c;
     if (which == 0) sincospi(-2.0 * (double)((long long)k * t % L) / (double)L, &s, &c);
     else sincospi(-2.0 * (double)((long long)(2 * k + 1) * t % (2 * L)) / (double)(2 * L), &s, &c);
@@ -35,13 +35,28 @@ __host__ __device__ inline int freq_of_pos(int pos, int N, int r1, int r2, int r
 }
 
 // Green's-spectrum axis table (Alg. 1 l.9-10, in FFT order rather than centred +
-// fftShift): p2[P] = (2 pi F~/(M dx))^2 / k0^2 with P = s*N + pos the position that
-// holds padded-grid frequency F = 2 freqN(pos) + s, F~ = F for F < M/2, F - M otherwise.
-__global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0) {
+// fftShift): p2[P] = (2 pi F~/(M dx))^2 / k0^2 for the padded-grid frequency F held at
+// index P of a transformed line, F~ = F for F < M/2, F - M otherwise.
+//   xorder = 0 (k_col lines): P = s*N + pos, F = 2 freqN(pos) + s.
+//   xorder = 1 (W rows, kernels.cuh): P = 2 q + s, q = k*(N/rl) + b, pos = b*rl + k.
+//   xorder = 2 (k_conv lines, read by the fused middle stage): P = s*N + k*(N/rl) + b, pos = b*rl + k.
+__global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0, int xorder) {
     const int P = blockIdx.x * blockDim.x + threadIdx.x;
     const int M = 2 * N;
     if (P >= M) return;
-    const int s = P / N, pos = P % N;
+    int s, pos;
+    if (xorder == 1) {
+        const int q = P >> 1, nbl = N / rl;
+        s = P & 1;
+        pos = (q % nbl) * rl + q / nbl;
+    } else if (xorder == 2) {
+        const int q = P % N, nbl = N / rl;
+        s = P / N;
+        pos = (q % nbl) * rl + q / nbl;
+    } else {
+        s = P / N;
+        pos = P % N;
+    }
     const int F = 2 * freq_of_pos(pos, N, r1, r2, rl) + s;
     const double Ft = (F < M / 2) ? (double)F : (double)(F - M);
     const double p = 2.0 * 3.14159265358979323846 * Ft / ((double)M * dx);

@@ -101,6 +101,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.ny = pl->n[1];
     a.rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
     a.src_scale = src_scale;
+    a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0));
     a.do_fwd = do_fwd;
     a.norms = pl->norms;
     a.history = pl->history;
@@ -123,8 +124,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
         a.in_line_stride = a.out_line_stride = mx;
         a.p2_line = f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
-        a.scale = (float)(1.0 / ((double)mx * (double)my));
-        if (which < 0 || which == 0) e = launch_col<MODE_CONV>(ny, a, 1, st);
+        if (which < 0 || which == 0) e = launch_conv(ny, a, 1, st);
         return e;
     }
     const long long mz = 2LL * nz;
@@ -134,7 +134,6 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = (long long)ny * mx; a.out_outer_stride = my * mx;
-        a.scale = 1.f;
         e = launch_col<MODE_FWD>(ny, a, nz, st);
         if (e != cudaSuccess) return e;
     }
@@ -145,8 +144,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
         a.p2_line = f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
-        a.scale = (float)(1.0 / ((double)mx * (double)my * (double)mz));
-        e = launch_col<MODE_CONV>(nz, a, (int)my, st);
+        e = launch_conv(nz, a, (int)my, st);
         if (e != cudaSuccess) return e;
     }
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
@@ -156,7 +154,6 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = my * mx; a.out_outer_stride = (long long)ny * mx;
         a.p2_line = nullptr; a.p2_inner = nullptr; a.p2_outer = nullptr;
-        a.scale = 1.f;
         e = launch_col<MODE_INV>(ny, a, nz, st);
     }
     return e;
@@ -178,10 +175,10 @@ cudaError_t set_kernel_attrs(tbs_plan *pl) {
     cudaError_t e;
     if ((e = launch_row<true>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
     if ((e = launch_row<false>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
-    if (pl->ndim == 2) return launch_col<MODE_CONV>(pl->n[1], ca, 1, 0, true);
+    if (pl->ndim == 2) return launch_conv(pl->n[1], ca, 1, 0, true);
     if ((e = launch_col<MODE_FWD>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
     if ((e = launch_col<MODE_INV>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
-    return launch_col<MODE_CONV>(pl->n[2], ca, 1, 0, true);
+    return launch_conv(pl->n[2], ca, 1, 0, true);
 }
 
 tbs_status ensure_history(tbs_plan *pl, int max_terms) {
@@ -304,7 +301,8 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
                 int r1, r2, rl;
                 radices_of(pl->n[a], r1, r2, rl);
                 CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
-                k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, dx_m, f.k0);
+                k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, dx_m, f.k0,
+                                                                 a == 0 ? 1 : (a == ndim - 1 ? 2 : 0));
             }
         }
         CU(pl, cudaDeviceSynchronize());
