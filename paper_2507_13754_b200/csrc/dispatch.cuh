@@ -31,13 +31,22 @@ template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 1; };
 
 // Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads.  Shared memory =
 // 2*T*(N + N/16 + 4)*8 bytes of work area + N*T*8 bytes of input staging.
-template <int N> struct ConvCfg { static constexpr int T = 16, MINB = 2; };    // N <= 256
+#ifndef TBS_CONV256_T
+#define TBS_CONV256_T 8
+#define TBS_CONV256_MINB 3
+#endif
+#ifndef TBS_CONV2048_T
+#define TBS_CONV2048_T 4
+#define TBS_CONV2048_MINB 1
+#endif
+template <int N> struct ConvCfg { static constexpr int T = 16, MINB = 2; };    // N < 256
+template <> struct ConvCfg<256>  { static constexpr int T = TBS_CONV256_T, MINB = TBS_CONV256_MINB; };
 template <> struct ConvCfg<512>  { static constexpr int T = 8, MINB = 2; };
 #ifndef TBS_CONV1024_T
 #define TBS_CONV1024_T 4
 #endif
 template <> struct ConvCfg<1024> { static constexpr int T = TBS_CONV1024_T, MINB = 2; };
-template <> struct ConvCfg<2048> { static constexpr int T = 4, MINB = 1; };
+template <> struct ConvCfg<2048> { static constexpr int T = TBS_CONV2048_T, MINB = TBS_CONV2048_MINB; };
 template <> struct ConvCfg<4096> { static constexpr int T = 2, MINB = 1; };
 
 // Persistent grids: number of CTAs that are resident at once (SMs x CTAs per SM), found once per
@@ -73,7 +82,7 @@ template <int N>
 static cudaError_t launch_conv_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = T * tpl_of(N);
-    constexpr size_t smem = (2 * (size_t)T * RowLay<N, conv_pad(N, T)>::PITCH + (size_t)N * T) * sizeof(float2);
+    constexpr size_t smem = (2 * (size_t)T * LineLay<N, conv_pad(N, T)>::PITCH + (size_t)N * T) * sizeof(float2);
     auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
     static int cap = 0;
     if (set_attr) {
@@ -123,7 +132,7 @@ static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr
     constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;
     constexpr int NT = C::GROUPS * TPL * GR;
     constexpr int ROWS = C::GROUPS * GR;
-    constexpr size_t smem = 2 * (size_t)ROWS * RowLay<N>::PITCH * sizeof(float2) +
+    constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
                             (FIRST ? 0 : (size_t)ROWS * N * sizeof(float4));
     auto kern = k_row<N, C::GROUPS, C::MINB, FIRST>;
     static int cap = 0;

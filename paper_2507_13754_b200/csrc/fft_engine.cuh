@@ -130,6 +130,7 @@ __device__ __forceinline__ void bfly(float2 (&v)[R]) {
 //   lutC[k][t] = w_S1^(k t)           middle stage (three-stage plans only)
 struct Luts {
     const float2 *A, *B, *C;
+    const float4 *AB;  // A and B interleaved (fft_engine_x2.cuh)
 };
 
 // K0 = 1 skips k = 0 (the twiddle is 1 in tables A and C).
@@ -193,11 +194,10 @@ struct RowLay {
 // Threads that own one line in the line-group kernels (k_row, k_conv): one radix-16 item each in
 // the widest stage.  Groups of TPL >= 32 threads synchronise on a named barrier of their own,
 // smaller groups share a warp and use __syncwarp, so no stage waits for the whole CTA.
-// Extra slots per line of the k_conv work area: the cooperative copy-out reads 2 chunks x 8 positions
-// (T = 4) or 4 chunks x 4 positions (T >= 8) per half-warp, conflict-free when the pitch is 4 resp.
-// 2 modulo 16.
+// Extra slots per line of the k_conv work area (16-byte slots): the cooperative copy-out reads, per
+// half-warp, 4 line pairs x 4 positions when T >= 8; a pitch of 2 modulo 8 spreads them evenly.
 __host__ __device__ constexpr int conv_pad(int N, int T) {
-    return ((T >= 8 ? 2 : 4) + 32 - (N + N / 16) % 16) % 16;
+    return T >= 8 ? (2 + 16 - (N + N / 16) % 8) % 8 : 0;
 }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
 template <int GT>
@@ -256,14 +256,6 @@ __device__ __forceinline__ void stage_pair(float2 *sm, const float2 *__restrict_
         stage_item<N, LB, R, FWD, Lay, HALF>(sm, lut, line, b);
     }
 }
-// one line, items dealt to the TPL threads that own it
-template <int N, int LB, int R, bool FWD, class Lay, int TPL, int HALF>
-__device__ __forceinline__ void stage_line(float2 *sm, const float2 *__restrict__ lut, int line, int lt) {
-    constexpr int NBL = N / R;
-#pragma unroll 1
-    for (int b = lt; b < NBL; b += TPL) stage_item<N, LB, R, FWD, Lay, HALF>(sm, lut, line, b);
-}
-
 // First forward stage from registers: x[j] is the input at position t + j*S1 (natural order).
 // Writes the even-frequency half (FFT of x) and the odd-frequency half (FFT of x w_2N^pos).
 template <int N, int R1, class Lay, int HALF>
@@ -324,52 +316,6 @@ __device__ __forceinline__ float rcp_fast(float d) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d));
     return r;
-}
-
-// Fused middle of the convolution: last forward stage (contiguous blocks of RL), multiply by
-// ghat, first inverse stage -- all in registers (north_star: "pointwise G multiply fused into the
-// last forward and first inverse butterfly stage").
-//   k0^2 ghat = 1/(a - i e) = (a + i e)/(a^2 + e^2),  a = a_line + p2[P],  e = eps/k0^2
-// (non-dimensional; the 1/prod(2N) of the inverse transforms is applied by k_row).
-template <int N, int RL, class Lay, int HALF>
-__device__ __forceinline__ void mid_conv_item(float2 *sm, int line, int b, const float *__restrict__ p2line,
-                                              float a_line, float e) {
-    const int base = b * RL;
-    const float e2 = e * e;
-#pragma unroll
-    for (int p = 0; p < 2; ++p) {
-        float2 *s = sm + p * HALF;
-        float2 v[RL];
-        float pp[RL];
-        // table in the transposed order [half][j][block]: consecutive threads, consecutive words
-#pragma unroll
-        for (int j = 0; j < RL; ++j) pp[j] = __ldg(p2line + p * N + j * (N / RL) + b);
-#pragma unroll
-        for (int j = 0; j < RL; ++j) v[j] = s[Lay::addr(line, base + j)];
-        bfly<RL, -1>(v);
-        float2 u[RL];
-#pragma unroll
-        for (int i = 0; i < RL; ++i) {
-            const int k = brev(i, RL);
-            const float a = a_line + pp[k];
-            const float r = rcp_fast(fmaf(a, a, e2));
-            const float tx = v[i].x * r, ty = v[i].y * r;
-            u[k] = make_float2(fmaf(tx, a, -ty * e), fmaf(tx, e, ty * a));
-        }
-        bfly<RL, +1>(u);
-#pragma unroll
-        for (int i = 0; i < RL; ++i) s[Lay::addr(line, base + brev(i, RL))] = u[i];
-    }
-}
-template <int N, int RL, class Lay, int NT, int HALF>
-__device__ __forceinline__ void mid_conv_pair(float2 *sm, int tid, int total, const float *__restrict__ p2line,
-                                              float a_line, float e) {
-    constexpr int NBL = N / RL;
-    for (int w = tid; w < total; w += NT) {
-        int line, b;
-        Lay::template split<NBL>(w, line, b);
-        mid_conv_item<N, RL, Lay, HALF>(sm, line, b, p2line, a_line, e);
-    }
 }
 
 }  // namespace tbs

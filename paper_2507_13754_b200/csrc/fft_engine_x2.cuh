@@ -1,0 +1,253 @@
+// fft_engine_x2.cuh -- the packed ("x2") form of the shared-memory FFT stages (sm_100a f32x2 pipe).
+//
+// The two parity halves of a zero-padded line (fft_engine.cuh: X[2k+s], s = 0, 1) go through the
+// same butterflies with the same twiddles at every stage, so they are carried as ONE value
+//   P2 = { re = (re_even, re_odd), im = (im_even, im_odd) }
+// and every add / multiply is a packed FADD2 / FMUL2 / FFMA2: half the issue slots of the scalar
+// form for the same FP32 results (the FP32 pipe itself is not wider: 128 results/clk/SM either way,
+// measured), and half the shared-memory instructions (one 16-byte access per position).  A scalar
+// twiddle is a broadcast operand and a negation an operand modifier, so no extra moves are issued.
+// Shared-memory element: float4 (re_even, re_odd, im_even, im_odd) per position.
+#pragma once
+#include "fft_engine.cuh"
+
+namespace tbs {
+
+struct P2 {
+    float2 re, im;
+};
+
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ P2 padd(P2 a, P2 b) { return P2{__fadd2_rn(a.re, b.re), __fadd2_rn(a.im, b.im)}; }
+__device__ __forceinline__ P2 psub(P2 a, P2 b) { return P2{__fadd2_rn(a.re, neg2(b.re)), __fadd2_rn(a.im, neg2(b.im))}; }
+// a * w, w a scalar complex (broadcast to both halves)
+__device__ __forceinline__ P2 pmul(P2 a, float2 w) {
+    return P2{__ffma2_rn(a.re, f2(w.x), __fmul2_rn(a.im, f2(-w.y))), __ffma2_rn(a.re, f2(w.y), __fmul2_rn(a.im, f2(w.x)))};
+}
+// a * conj(w)
+__device__ __forceinline__ P2 pmulc(P2 a, float2 w) {
+    return P2{__ffma2_rn(a.re, f2(w.x), __fmul2_rn(a.im, f2(w.y))), __ffma2_rn(a.im, f2(w.x), __fmul2_rn(a.re, f2(-w.y)))};
+}
+// a * w, w = (wre, wim) a different twiddle per half
+__device__ __forceinline__ P2 pmul2(P2 a, float2 wre, float2 wim) {
+    return P2{__ffma2_rn(a.re, wre, __fmul2_rn(a.im, neg2(wim))), __ffma2_rn(a.re, wim, __fmul2_rn(a.im, wre))};
+}
+__device__ __forceinline__ P2 pmulc2(P2 a, float2 wre, float2 wim) {
+    return P2{__ffma2_rn(a.re, wre, __fmul2_rn(a.im, wim)), __ffma2_rn(a.im, wre, __fmul2_rn(a.re, neg2(wim)))};
+}
+
+// d * w_16^(idx16) with sign SGN, both halves (packed form of mul_w16).
+template <int SGN>
+__device__ __forceinline__ P2 pmul_w16(P2 d, int idx16) {
+    constexpr float C1 = 0.92387953251128674f;  // cos(pi/8)
+    constexpr float S1 = 0.38268343236508977f;  // sin(pi/8)
+    constexpr float H = 0.70710678118654752f;   // sqrt(1/2)
+    constexpr float s = (float)SGN;
+    switch (idx16) {
+        case 0: return d;
+        case 1: return pmul(d, make_float2(C1, s * S1));
+        case 2: return P2{__fmul2_rn(__fadd2_rn(d.re, SGN > 0 ? neg2(d.im) : d.im), f2(H)),
+                          __fmul2_rn(__fadd2_rn(d.im, SGN > 0 ? d.re : neg2(d.re)), f2(H))};
+        case 3: return pmul(d, make_float2(S1, s * C1));
+        case 4: return SGN > 0 ? P2{neg2(d.im), d.re} : P2{d.im, neg2(d.re)};
+        case 5: return pmul(d, make_float2(-S1, s * C1));
+        case 6: return P2{__fmul2_rn(__fadd2_rn(neg2(d.re), SGN > 0 ? neg2(d.im) : d.im), f2(H)),
+                          __fmul2_rn(__fadd2_rn(neg2(d.im), SGN > 0 ? d.re : neg2(d.re)), f2(H))};
+        default: return pmul(d, make_float2(-C1, s * S1));
+    }
+}
+
+// DFT_R of v (sign SGN), natural order in, BIT-REVERSED order out, both halves at once.
+template <int R, int SGN>
+__device__ __forceinline__ void pbfly(P2 (&v)[R]) {
+#pragma unroll
+    for (int h = R / 2; h >= 1; h >>= 1) {
+#pragma unroll
+        for (int g = 0; g < R; g += 2 * h) {
+#pragma unroll
+            for (int m = 0; m < h; ++m) {
+                const P2 a = v[g + m], b = v[g + m + h];
+                v[g + m] = padd(a, b);
+                v[g + m + h] = pmul_w16<SGN>(psub(a, b), m * (8 / h));
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ P2 lds_p2(const float4 *p) {
+    const float4 f = *p;
+    return P2{make_float2(f.x, f.y), make_float2(f.z, f.w)};
+}
+__device__ __forceinline__ void sts_p2(float4 *p, P2 v) { *p = make_float4(v.re.x, v.re.y, v.im.x, v.im.y); }
+
+// Packed line layout: one float4 per position, one pad slot per 16 positions, PAD extra per line.
+template <int N, int PAD = 0>
+struct LineLay {
+    static constexpr int PITCH = N + N / 16 + PAD;
+    __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + pos + (pos >> 4); }
+};
+
+// In-place stage (block length LB, radix R, sub-stride S = LB/R) of one item of one line.
+// FWD (DIF): butterfly then twiddle w_LB^(k t);  inverse (DIT): conj twiddle then butterfly.
+template <int N, int LB, int R, bool FWD, class Lay>
+__device__ __forceinline__ void pstage_item_tw(float4 *sm, const float2 (&tw)[R], int line, int b) {
+    constexpr int S = LB / R;
+    const int t = b % S;
+    const int base = (b / S) * LB + t;
+    P2 v[R];
+    if (FWD) {
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j * S));
+                pbfly<R, -1>(v);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int k = brev(i, R);
+            if (S > 1 && k > 0) v[i] = pmul(v[i], tw[k]);
+        }
+    #pragma unroll
+        for (int i = 0; i < R; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, R) * S), v[i]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = lds_p2(sm + Lay::addr(line, base + k * S));
+    #pragma unroll
+        for (int k = 0; k < R; ++k)
+            if (S > 1 && k > 0) v[k] = pmulc(v[k], tw[k]);
+        pbfly<R, +1>(v);
+#pragma unroll
+        for (int i = 0; i < R; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, R) * S), v[i]);
+    }
+}
+template <int N, int LB, int R, bool FWD, class Lay>
+__device__ __forceinline__ void pstage_item(float4 *sm, const float2 *__restrict__ lut, int line, int b) {
+    constexpr int S = LB / R;
+    float2 tw[R];
+    if (S > 1) load_tw<R, S, 1>(tw, lut, b % S);
+    pstage_item_tw<N, LB, R, FWD, Lay>(sm, tw, line, b);
+}
+// The same with the twiddles of the thread's first item already in registers (fetched before the
+// barrier that precedes the stage, so that their L2 latency is not exposed after it).
+template <int N, int LB, int R, bool FWD, class Lay, int TPL>
+__device__ __forceinline__ void pstage_line_pre(float4 *sm, const float2 *__restrict__ lut, float2 (&tw)[R], int line, int lt) {
+    constexpr int S = LB / R, NBL = N / R;
+#pragma unroll 1
+    for (int b = lt; b < NBL; b += TPL) {
+        if (b != lt && S > 1) load_tw<R, S, 1>(tw, lut, b % S);
+        pstage_item_tw<N, LB, R, FWD, Lay>(sm, tw, line, b);
+    }
+}
+template <int N, int LB, int R, bool FWD, class Lay, int TPL>
+__device__ __forceinline__ void pstage_line(float4 *sm, const float2 *__restrict__ lut, int line, int lt) {
+    constexpr int NBL = N / R;
+#pragma unroll 1
+    for (int b = lt; b < NBL; b += TPL) pstage_item<N, LB, R, FWD, Lay>(sm, lut, line, b);
+}
+
+// Interleaved first/last-stage table: lutAB[k][t] = (A.x, B.x, A.y, B.y) with A = w_N^(k t) (even
+// half) and B = w_2N^((2k+1) t) (odd half, carries the zero-padding twist; fft_engine.cuh).
+template <int R, int S>
+__device__ __forceinline__ void load_tw_ab(float2 (&wre)[R], float2 (&wim)[R], const float4 *__restrict__ lut, int t) {
+#pragma unroll
+    for (int k = 0; k < R; ++k) {
+        const float4 f = __ldg(lut + k * S + t);
+        wre[k] = make_float2(f.x, f.y);
+        wim[k] = make_float2(f.z, f.w);
+    }
+}
+
+// First forward stage from registers: x[j] is the input at position t + j*S1 (natural order).
+// even half: FFT of x; odd half: FFT of x w_2N^pos (the constant part w_(2 R1)^j applied here).
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void pfirst_fwd_tw(const float2 (&x)[R1], int line, int t, float4 *sm,
+                                              const float2 (&wre)[R1], const float2 (&wim)[R1]) {
+    constexpr int S1 = N / R1;
+    P2 v[R1];
+#pragma unroll
+    for (int j = 0; j < R1; ++j) {
+        const float2 o = j > 0 ? mul_w32<-1>(x[j], j * (16 / R1)) : x[j];
+        v[j] = P2{make_float2(x[j].x, o.x), make_float2(x[j].y, o.y)};
+    }
+    pbfly<R1, -1>(v);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) v[i] = pmul2(v[i], wre[brev(i, R1)], wim[brev(i, R1)]);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) sts_p2(sm + Lay::addr(line, t + brev(i, R1) * S1), v[i]);
+}
+
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void pfirst_fwd(const float2 (&x)[R1], int line, int t, float4 *sm,
+                                           const float4 *__restrict__ lutAB) {
+    float2 wre[R1], wim[R1];
+    load_tw_ab<R1, N / R1>(wre, wim, lutAB, t);
+    pfirst_fwd_tw<N, R1, Lay>(x, line, t, sm, wre, wim);
+}
+
+// Last inverse stage into registers, both halves combined (inverse of pfirst_fwd followed by the
+// crop): z[j] = IFFT_N(even half)[pos] + conj(w_2N^pos) IFFT_N(odd half)[pos], pos = t + j*S1.
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void plast_inv_tw(float2 (&z)[R1], int line, int t, const float4 *sm,
+                                             const float2 (&wre)[R1], const float2 (&wim)[R1]) {
+    constexpr int S1 = N / R1;
+    P2 v[R1];
+#pragma unroll
+    for (int k = 0; k < R1; ++k) v[k] = lds_p2(sm + Lay::addr(line, t + k * S1));
+#pragma unroll
+    for (int k = 0; k < R1; ++k) v[k] = pmulc2(v[k], wre[k], wim[k]);
+    pbfly<R1, +1>(v);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) {
+        const int j = brev(i, R1);
+        const float2 o = mul_w32<+1>(make_float2(v[i].re.y, v[i].im.y), j * (16 / R1));
+        z[j] = make_float2(v[i].re.x + o.x, v[i].im.x + o.y);
+    }
+}
+
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void plast_inv(float2 (&z)[R1], int line, int t, const float4 *sm,
+                                          const float4 *__restrict__ lutAB) {
+    float2 wre[R1], wim[R1];
+    load_tw_ab<R1, N / R1>(wre, wim, lutAB, t);
+    plast_inv_tw<N, R1, Lay>(z, line, t, sm, wre, wim);
+}
+
+// Fused middle of the convolution (packed form of mid_conv_item): last forward stage (contiguous
+// blocks of RL), multiply by ghat, first inverse stage, in registers.
+//   k0^2 ghat = (a + i e)/(a^2 + e^2),  a = a_line + p2[half][P],  e = eps/k0^2
+// p2x2: the line-axis table interleaved over the halves, [j][block] float2 = (even, odd).
+template <int N, int RL>
+__device__ __forceinline__ void load_p2x2(float2 (&pp)[RL], const float2 *__restrict__ p2x2, int b) {
+#pragma unroll
+    for (int j = 0; j < RL; ++j) pp[j] = __ldg(p2x2 + j * (N / RL) + b);
+}
+template <int N, int RL, class Lay>
+__device__ __forceinline__ void pmid_conv_item_pp(float4 *sm, int line, int b, const float2 (&pp)[RL],
+                                                  float a_line, float e) {
+    const int base = b * RL;
+    const float e2 = e * e;
+    P2 v[RL];
+#pragma unroll
+    for (int j = 0; j < RL; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j));
+    pbfly<RL, -1>(v);
+    P2 u[RL];
+#pragma unroll
+    for (int i = 0; i < RL; ++i) {
+        const int k = brev(i, RL);
+        const float2 a = __fadd2_rn(pp[k], f2(a_line));
+        const float2 d = __ffma2_rn(a, a, f2(e2));
+        const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
+        const float2 tx = __fmul2_rn(v[i].re, r), ty = __fmul2_rn(v[i].im, r);
+        u[k] = P2{__ffma2_rn(tx, a, __fmul2_rn(ty, f2(-e))), __ffma2_rn(tx, f2(e), __fmul2_rn(ty, a))};
+    }
+    pbfly<RL, +1>(u);
+#pragma unroll
+    for (int i = 0; i < RL; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, RL)), u[i]);
+}
+template <int N, int RL, class Lay>
+__device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
+                                               float a_line, float e) {
+    float2 pp[RL];
+    load_p2x2<N, RL>(pp, p2x2, b);
+    pmid_conv_item_pp<N, RL, Lay>(sm, line, b, pp, a_line, e);
+}
+
+}  // namespace tbs

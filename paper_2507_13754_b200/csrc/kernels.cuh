@@ -12,7 +12,7 @@
 // Both parity halves of a padded line (fft_engine.cuh) are resident in shared memory at once, so
 // the input is read once and the twiddles of a butterfly pair are fetched once.
 #pragma once
-#include "fft_engine.cuh"
+#include "fft_engine_x2.cuh"
 
 namespace tbs {
 
@@ -36,7 +36,7 @@ struct ColArgs {
     long long in_outer_stride, out_outer_stride;  // between consecutive outer indices
     int inner_len;                                // number of adjacent lines (multiple of T)
     int n_outer;                                  // number of outer indices
-    const float *p2_line;   // [2N] |p|^2/k0^2 of this axis, position order       (CONV)
+    const float2 *p2_line;  // [N] (even, odd) |p|^2/k0^2 of the line axis, order of pmid_conv_item
     const float *p2_inner;  // [inner_len] of the inner (x) axis, position order  (CONV)
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
     float e;                // eps/k0^2                                           (CONV)
@@ -205,10 +205,10 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     constexpr int GT = TPL * GR;                   // threads per group
     constexpr int NT = GROUPS * GT;
     constexpr int ROWS = GROUPS * GR;
-    using Lay = RowLay<N>;
-    constexpr int HALF = ROWS * Lay::PITCH;
+    using Lay = LineLay<N>;
     extern __shared__ __align__(128) float2 sm[];
-    float4 *stg = reinterpret_cast<float4 *>(sm + 2 * HALF);  // [ROWS][N] staged W rows
+    float4 *wk = reinterpret_cast<float4 *>(sm);  // [ROWS][PITCH] work area, both halves per slot
+    float4 *stg = wk + ROWS * Lay::PITCH;         // [ROWS][N] staged W rows
     __shared__ float red[2][32];
     __shared__ __align__(8) uint64_t mbar[GROUPS];
     if (a.ctl->done) return;
@@ -223,6 +223,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     constexpr uint32_t TILE_BYTES = (uint32_t)GR * M * sizeof(float2);
     uint32_t phase = 0;
     float uu = 0.f, pp = 0.f;
+
     int gt = blockIdx.x * GROUPS + g;
     if (!FIRST) {
         if (tid == 0)
@@ -252,19 +253,15 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             // first inverse stage (contiguous blocks of RL) from the staged rows
 #pragma unroll 1
             for (int b = lt; b < NBL; b += TPL) {
-                float2 v0[RL], v1[RL];
+                P2 v[RL];
 #pragma unroll
                 for (int k = 0; k < RL; ++k) {
                     const float4 f = stg[l * N + k * NBL + b];
-                    v0[k] = make_float2(f.x, f.y);
-                    v1[k] = make_float2(f.z, f.w);
+                    v[k] = P2{make_float2(f.x, f.z), make_float2(f.y, f.w)};
                 }
-                bfly<RL, +1>(v0);
+                pbfly<RL, +1>(v);
 #pragma unroll
-                for (int i = 0; i < RL; ++i) sm[Lay::addr(l, b * RL + brev(i, RL))] = v0[i];
-                bfly<RL, +1>(v1);
-#pragma unroll
-                for (int i = 0; i < RL; ++i) sm[HALF + Lay::addr(l, b * RL + brev(i, RL))] = v1[i];
+                for (int i = 0; i < RL; ++i) sts_p2(wk + Lay::addr(l, b * RL + brev(i, RL)), v[i]);
             }
             group_sync<GT>(g);
             // the group's staging rows are free: fetch the W rows of its next tile
@@ -273,7 +270,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 bulk_g2s(stg + g * GR * N, a.W + (long long)(gt + gstride) * GR * M, TILE_BYTES, &mbar[g]);
             }
             if (R2 > 0) {
-                stage_line<N, S1, R2s, false, Lay, TPL, HALF>(sm, a.lut.C, l, lt);
+                pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
                 group_sync<GT>(g);
             }
         }
@@ -283,7 +280,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
         for (int t = lt; t < S1; t += TPL) {
             float2 x[R1];
             if (!FIRST) {
-                last_inv_pair<N, R1, Lay, HALF>(x, l, t, sm, a.lut);
+                plast_inv<N, R1, Lay>(x, l, t, wk, a.lut.AB);
 #pragma unroll
                 for (int j = 0; j < R1; ++j) {
                     const int pos = t + j * S1;
@@ -305,30 +302,27 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     x[j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
                 }
             }
-            first_fwd_pair<N, R1, Lay, HALF>(x, l, t, sm, a.lut);
+            pfirst_fwd<N, R1, Lay>(x, l, t, wk, a.lut.AB);
         }
         group_sync<GT>(g);
         if (!FIRST && !a.do_fwd) continue;
         // ---------------- forward half: the remaining stages of FFT_x ----------------
         if (R2 > 0) {
-            stage_line<N, S1, R2s, true, Lay, TPL, HALF>(sm, a.lut.C, l, lt);
+            pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, l, lt);
             group_sync<GT>(g);
         }
         // last forward stage (contiguous blocks of RL) straight to global memory.  A thread reads
         // exactly the slots it writes in the first inverse stage of its next tile.
 #pragma unroll 1
         for (int b = lt; b < NBL; b += TPL) {
-            float2 v0[RL], v1[RL];
+            P2 v[RL];
 #pragma unroll
-            for (int j = 0; j < RL; ++j) v0[j] = sm[Lay::addr(l, b * RL + j)];
-            bfly<RL, -1>(v0);
-#pragma unroll
-            for (int j = 0; j < RL; ++j) v1[j] = sm[HALF + Lay::addr(l, b * RL + j)];
-            bfly<RL, -1>(v1);
+            for (int j = 0; j < RL; ++j) v[j] = lds_p2(wk + Lay::addr(l, b * RL + j));
+            pbfly<RL, -1>(v);
             float4 *gp = reinterpret_cast<float4 *>(a.W + (long long)row * M) + b;
 #pragma unroll
             for (int i = 0; i < RL; ++i)
-                gp[brev(i, RL) * NBL] = make_float4(v0[i].x, v0[i].y, v1[i].x, v1[i].y);
+                gp[brev(i, RL) * NBL] = make_float4(v[i].re.x, v[i].im.x, v[i].re.y, v[i].im.y);
         }
         if (FIRST) group_sync<GT>(g);  // the next tile's first stage writes slots other threads still read
     }
@@ -387,13 +381,13 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
     constexpr int GT = TPL >= 32 ? TPL : 32;
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
-    using Lay = RowLay<N, conv_pad(N, T)>;
-    constexpr int HALF = T * Lay::PITCH;
+    using Lay = LineLay<N, conv_pad(N, T)>;
     extern __shared__ __align__(128) float2 sm[];
+    float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
     // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
     // 2c+1), the chunk index XOR-swizzled with the position so that the cp.async writes of a warp are
     // contiguous and the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
-    float4 *stg = reinterpret_cast<float4 *>(sm + 2 * HALF);
+    float4 *stg = wk + T * Lay::PITCH;
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
@@ -403,13 +397,21 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
     const int total = tiles * a.n_outer;
     auto swz = [](int r) { return CPR > 1 ? (r / (CPR >= 8 ? 1 : 8 / CPR)) % CPR : 0; };
 
-    auto stage_tile = [&](int tile) {
+    // part q of NQ of the cp.async copies of one tile (spread over the phases of the previous tile)
+    constexpr int NQ = 4;
+    static_assert((N * CPR) % (NT * NQ) == 0 || N * CPR < NT * NQ, "staging split");
+    auto stage_part = [&](int tile, int q) {
         const float2 *src = a.in + (long long)(tile / tiles) * a.in_outer_stride + (tile % tiles) * T;
-#pragma unroll 4
-        for (int c = tid; c < N * CPR; c += NT) {
+        constexpr int PER = (N * CPR + NQ - 1) / NQ;
+#pragma unroll 2
+        for (int c = q * PER + tid; c < (q + 1) * PER && c < N * CPR; c += NT) {
             const int r = c / CPR, cc = c % CPR;
             cp_async16(stg + r * CPR + (cc ^ swz(r)), src + (long long)r * a.in_line_stride + 2 * cc);
         }
+    };
+    auto stage_tile = [&](int tile) {
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) stage_part(tile, q);
         cp_async_commit();
     };
     if ((int)blockIdx.x < total) stage_tile(blockIdx.x);
@@ -419,6 +421,7 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
     for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
         const int inner0 = (tile % tiles) * T;
         const int outer = tile / tiles;
+        const bool more = tile + (int)gridDim.x < total;
         cp_async_wait_all();
         __syncthreads();  // staged tile visible; the copy-out of the previous tile has left the work area
         // ---- forward: N inputs -> both halves ----
@@ -430,32 +433,41 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
                 const int r = t + j * S1;
                 x[j] = stg2[2 * (r * CPR + ((line >> 1) ^ swz(r)))];
             }
-            first_fwd_pair<N, R1, Lay, HALF>(x, line, t, sm, a.lut);
+            pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
         }
         __syncthreads();  // staging buffer free (and the line groups are in step)
-        if (tile + (int)gridDim.x < total) stage_tile(tile + gridDim.x);
+        // the cp.async copies of the next tile are issued in four parts, one after each stage
+        if (more) stage_part(tile + gridDim.x, 0);
         if (R2 > 0) {
-            stage_line<N, S1, R2s, true, Lay, TPL, HALF>(sm, a.lut.C, line, lt);
+            pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, line, lt);
             group_sync<GT>(g);
         }
         {
             float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
             if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) mid_conv_item<N, RL, Lay, HALF>(sm, line, b, a.p2_line, a_line, a.e);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line, a.e);
+            if (more) stage_part(tile + gridDim.x, 1);
             group_sync<GT>(g);
         }
-        // ---- inverse: both halves -> N outputs, left in the even half of the work area ----
+        // ---- inverse: both halves -> N outputs, left in the first 8 bytes of their slots ----
         if (R2 > 0) {
-            stage_line<N, S1, R2s, false, Lay, TPL, HALF>(sm, a.lut.C, line, lt);
+            pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, line, lt);
+            if (more) stage_part(tile + gridDim.x, 2);
             group_sync<GT>(g);
+        } else if (more) {
+            stage_part(tile + gridDim.x, 2);
         }
 #pragma unroll 1
         for (int t = lt; t < S1; t += TPL) {
             float2 z[R1];
-            last_inv_pair<N, R1, Lay, HALF>(z, line, t, sm, a.lut);
+            plast_inv<N, R1, Lay>(z, line, t, wk, a.lut.AB);
 #pragma unroll
-            for (int j = 0; j < R1; ++j) sm[Lay::addr(line, t + j * S1)] = z[j];
+            for (int j = 0; j < R1; ++j) *reinterpret_cast<float2 *>(wk + Lay::addr(line, t + j * S1)) = z[j];
+        }
+        if (more) {
+            stage_part(tile + gridDim.x, 3);
+            cp_async_commit();
         }
         __syncthreads();
         float2 *dst = a.out + (long long)outer * a.out_outer_stride + inner0;
@@ -464,7 +476,8 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
 #pragma unroll 4
         for (int c = tid; c < N * CPR; c += NT) {
             const int r = (c / CL) % N, cc = (c / (CL * N)) * CL + c % CL;
-            const float2 v0 = sm[Lay::addr(2 * cc, r)], v1 = sm[Lay::addr(2 * cc + 1, r)];
+            const float2 v0 = *reinterpret_cast<const float2 *>(wk + Lay::addr(2 * cc, r));
+            const float2 v1 = *reinterpret_cast<const float2 *>(wk + Lay::addr(2 * cc + 1, r));
             *reinterpret_cast<float4 *>(dst + (long long)r * a.out_line_stride + 2 * cc) = make_float4(v0.x, v0.y, v1.x, v1.y);
         }
     }

@@ -20,6 +20,19 @@ __global__ void k_stage_lut(float2 *lut, int L, int R, int which) {
     lut[i] = make_float2((float)c, (float)s);
 }
 
+// First/last-stage tables A and B interleaved for the packed engine (fft_engine_x2.cuh):
+// lut[k][t] = (A.x, B.x, A.y, B.y), A = exp(-2 pi i k t / N), B = exp(-2 pi i (2k+1) t / (2N)).
+__global__ void k_stage_lut_ab(float4 *lut, int N, int R) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int S = N / R;
+    if (i >= S * R) return;
+    const int k = i / S, t = i % S;
+    double sa, ca, sb, cb;
+    sincospi(-2.0 * (double)((long long)k * t % N) / (double)N, &sa, &ca);
+    sincospi(-2.0 * (double)((long long)(2 * k + 1) * t % (2 * N)) / (double)(2 * N), &sb, &cb);
+    lut[i] = make_float4((float)ca, (float)cb, (float)sa, (float)sb);
+}
+
 // Frequency index held at `pos` of a length-N DIF transform with radices r1, r2 (0 = none), rl.
 __host__ __device__ inline int freq_of_pos(int pos, int N, int r1, int r2, int rl) {
     const int s1 = N / r1;
@@ -38,20 +51,16 @@ __host__ __device__ inline int freq_of_pos(int pos, int N, int r1, int r2, int r
 // fftShift): p2[P] = (2 pi F~/(M dx))^2 / k0^2 for the padded-grid frequency F held at
 // index P of a transformed line, F~ = F for F < M/2, F - M otherwise.
 //   xorder = 0 (k_col lines): P = s*N + pos, F = 2 freqN(pos) + s.
-//   xorder = 1 (W rows, kernels.cuh): P = 2 q + s, q = k*(N/rl) + b, pos = b*rl + k.
-//   xorder = 2 (k_conv lines, read by the fused middle stage): P = s*N + k*(N/rl) + b, pos = b*rl + k.
+//   xorder = 1 (W rows of k_row; line-axis table of k_conv's fused middle stage):
+//                P = 2 q + s, q = k*(N/rl) + b, pos = b*rl + k.
 __global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0, int xorder) {
     const int P = blockIdx.x * blockDim.x + threadIdx.x;
     const int M = 2 * N;
     if (P >= M) return;
     int s, pos;
-    if (xorder == 1) {
+    if (xorder) {
         const int q = P >> 1, nbl = N / rl;
         s = P & 1;
-        pos = (q % nbl) * rl + q / nbl;
-    } else if (xorder == 2) {
-        const int q = P % N, nbl = N / rl;
-        s = P / N;
         pos = (q % nbl) * rl + q / nbl;
     } else {
         s = P / N;

@@ -42,6 +42,7 @@ struct tbs_plan {
     float2 *lutA[3] = {nullptr, nullptr, nullptr};   // per axis, fft_engine.cuh "Luts"
     float2 *lutB[3] = {nullptr, nullptr, nullptr};
     float2 *lutC[3] = {nullptr, nullptr, nullptr};
+    float4 *lutAB[3] = {nullptr, nullptr, nullptr};
     float2 *W1 = nullptr;   // [nz*ny][2 nx]
     float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]
     float *abl[3] = {nullptr, nullptr, nullptr};
@@ -106,7 +107,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.norms = pl->norms;
     a.history = pl->history;
     a.ctl = f.ctl;
-    a.lut = Luts{pl->lutA[0], pl->lutB[0], pl->lutC[0]};
+    a.lut = Luts{pl->lutA[0], pl->lutB[0], pl->lutC[0], pl->lutAB[0]};
 }
 
 // Column / plane passes of one term (K2 in 2-D; y-forward, z-conv, y-inverse in 3-D).
@@ -121,9 +122,9 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
         a.in = pl->W1; a.out = pl->W1;
-        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = a.out_line_stride = mx;
-        a.p2_line = f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
+        a.p2_line = (const float2 *)f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
         if (which < 0 || which == 0) e = launch_conv(ny, a, 1, st);
         return e;
     }
@@ -131,7 +132,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
     if (which < 0 || which == 0) {
         a.in = pl->W1; a.out = pl->W2;
-        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = (long long)ny * mx; a.out_outer_stride = my * mx;
         e = launch_col<MODE_FWD>(ny, a, nz, st);
@@ -140,17 +141,17 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     // z convolution, in place on W2; lines (ky, kx), outer = ky
     if (which < 0 || which == 1) {
         a.in = pl->W2; a.out = pl->W2;
-        a.lut = Luts{pl->lutA[2], pl->lutB[2], pl->lutC[2]};
+        a.lut = Luts{pl->lutA[2], pl->lutB[2], pl->lutC[2], pl->lutAB[2]};
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
-        a.p2_line = f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
+        a.p2_line = (const float2 *)f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
         e = launch_conv(nz, a, (int)my, st);
         if (e != cudaSuccess) return e;
     }
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
     if (which < 0 || which == 2) {
         a.in = pl->W2; a.out = pl->W1;
-        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1]};
+        a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = my * mx; a.out_outer_stride = (long long)ny * mx;
         a.p2_line = nullptr; a.p2_inner = nullptr; a.p2_outer = nullptr;
@@ -228,7 +229,7 @@ void tbs_plan_destroy(tbs_plan *pl) {
         cudaFree(f.V); cudaFree(f.S); cudaFree(f.p); cudaFree(f.ctl);
         for (int a = 0; a < 3; ++a) cudaFree(f.p2[a]);
     }
-    for (int a = 0; a < 3; ++a) { cudaFree(pl->lutA[a]); cudaFree(pl->lutB[a]); cudaFree(pl->lutC[a]); }
+    for (int a = 0; a < 3; ++a) { cudaFree(pl->lutA[a]); cudaFree(pl->lutB[a]); cudaFree(pl->lutC[a]); cudaFree(pl->lutAB[a]); }
     cudaFree(pl->W1); cudaFree(pl->W2);
     for (int a = 0; a < 3; ++a) cudaFree(pl->abl[a]);
     cudaFree(pl->norms); cudaFree(pl->history); cudaFree(pl->maxbits);
@@ -271,6 +272,8 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
             CU(pl, dmalloc(pl, &pl->lutB[a], N));
             k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutA[a], N, r1, 0);
             k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutB[a], N, r1, 1);
+            CU(pl, dmalloc(pl, &pl->lutAB[a], N));
+            k_stage_lut_ab<<<nblk(N, 256), 256>>>(pl->lutAB[a], N, r1);
             if (r2 > 0) {
                 CU(pl, dmalloc(pl, &pl->lutC[a], N / r1));
                 k_stage_lut<<<nblk(N / r1, 256), 256>>>(pl->lutC[a], N / r1, r2, 0);
@@ -302,7 +305,7 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
                 radices_of(pl->n[a], r1, r2, rl);
                 CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
                 k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, dx_m, f.k0,
-                                                                 a == 0 ? 1 : (a == ndim - 1 ? 2 : 0));
+                                                                 a == 0 || a == ndim - 1);
             }
         }
         CU(pl, cudaDeviceSynchronize());
