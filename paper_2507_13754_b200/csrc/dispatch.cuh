@@ -4,8 +4,8 @@
 
 namespace tbs {
 
-// Column-tile kernel k_col (3-D y passes, N <= 512): T adjacent lines per CTA, NT threads.  Shared memory = 2*N*T*8 bytes
-// (both parity halves of the padded line) + N*T*8 bytes of input staging (CONV, FWD).
+// Column-tile kernel k_col (3-D y passes): T adjacent lines per CTA, NT threads.  Shared memory =
+// 2*N*T*8 bytes (both parity halves of the padded line) + N*T*8 bytes of input staging (FWD).
 template <int N> struct ColCfg;
 template <> struct ColCfg<32>   { static constexpr int T = 16, NT = 64;  };
 template <> struct ColCfg<64>   { static constexpr int T = 16, NT = 128; };
@@ -13,40 +13,21 @@ template <> struct ColCfg<128>  { static constexpr int T = 16, NT = 128; };
 template <> struct ColCfg<256>  { static constexpr int T = 16, NT = 256; };
 template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
 
-// Row kernel: GROUPS independent line groups per CTA (a group = N/16 threads on one row, or one warp
-// on 32/(N/16) rows), at least MINB CTAs per SM (register cap).  Shared memory per row =
-// 2*(N + N/16)*8 bytes of work area + N*16 bytes of W staging.
-template <int N> struct RowCfg { static constexpr int GROUPS = 4, MINB = 3; };   // N <= 512
-#ifndef TBS_ROW1024_GROUPS
-#define TBS_ROW1024_GROUPS 2
-#define TBS_ROW1024_MINB 3
-#endif
-#ifndef TBS_ROW2048_GROUPS
-#define TBS_ROW2048_GROUPS 1
-#define TBS_ROW2048_MINB 3
-#endif
-template <> struct RowCfg<1024> { static constexpr int GROUPS = TBS_ROW1024_GROUPS, MINB = TBS_ROW1024_MINB; };
-template <> struct RowCfg<2048> { static constexpr int GROUPS = TBS_ROW2048_GROUPS, MINB = TBS_ROW2048_MINB; };
+// Row kernel k_row: GROUPS independent line groups per CTA (a group = N/16 threads on one row, or
+// one warp on 32/(N/16) rows), at least MINB CTAs per SM (register cap).  Shared memory per row =
+// (N + N/16)*16 bytes of work area + N*16 bytes of W staging.  Values measured on B200 (cfg2-cfg5).
+template <int N> struct RowCfg { static constexpr int GROUPS = 4, MINB = 2; };   // N <= 512
+template <> struct RowCfg<1024> { static constexpr int GROUPS = 2, MINB = 3; };
+template <> struct RowCfg<2048> { static constexpr int GROUPS = 1, MINB = 3; };
 template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 1; };
 
-// Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads.  Shared memory =
-// 2*T*(N + N/16 + 4)*8 bytes of work area + N*T*8 bytes of input staging.
-#ifndef TBS_CONV256_T
-#define TBS_CONV256_T 8
-#define TBS_CONV256_MINB 3
-#endif
-#ifndef TBS_CONV2048_T
-#define TBS_CONV2048_T 4
-#define TBS_CONV2048_MINB 1
-#endif
+// Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads, at least MINB CTAs
+// per SM.  Shared memory = T*(N + N/16 + pad)*16 bytes of work area + N*T*8 bytes of input staging.
 template <int N> struct ConvCfg { static constexpr int T = 16, MINB = 2; };    // N < 256
-template <> struct ConvCfg<256>  { static constexpr int T = TBS_CONV256_T, MINB = TBS_CONV256_MINB; };
+template <> struct ConvCfg<256>  { static constexpr int T = 8, MINB = 3; };
 template <> struct ConvCfg<512>  { static constexpr int T = 8, MINB = 2; };
-#ifndef TBS_CONV1024_T
-#define TBS_CONV1024_T 4
-#endif
-template <> struct ConvCfg<1024> { static constexpr int T = TBS_CONV1024_T, MINB = 2; };
-template <> struct ConvCfg<2048> { static constexpr int T = TBS_CONV2048_T, MINB = TBS_CONV2048_MINB; };
+template <> struct ConvCfg<1024> { static constexpr int T = 4, MINB = 2; };
+template <> struct ConvCfg<2048> { static constexpr int T = 4, MINB = 1; };
 template <> struct ConvCfg<4096> { static constexpr int T = 2, MINB = 1; };
 
 // Persistent grids: number of CTAs that are resident at once (SMs x CTAs per SM), found once per

@@ -205,6 +205,8 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     constexpr int GT = TPL * GR;                   // threads per group
     constexpr int NT = GROUPS * GT;
     constexpr int ROWS = GROUPS * GR;
+    constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
+    static_assert(S1 % TPL == 0, "items per thread");
     using Lay = LineLay<N>;
     extern __shared__ __align__(128) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [ROWS][PITCH] work area, both halves per slot
@@ -239,6 +241,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     for (; gt < ngt; gt += gstride) {
         const int row = gt * GR + gl / TPL;
         float wrow = a.scale;
+        float2 pold[NITEM][R1], vpot[NITEM][R1];
         if (!FIRST) {
             // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
             // pull the p and V rows of this tile towards L2 while the W rows arrive
@@ -269,30 +272,41 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 mbar_expect_tx(&mbar[g], TILE_BYTES);
                 bulk_g2s(stg + g * GR * N, a.W + (long long)(gt + gstride) * GR * M, TILE_BYTES, &mbar[g]);
             }
-            if (R2 > 0) {
-                pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
-                group_sync<GT>(g);
-            }
+            if (R2 > 0) pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
+            // request the running field and the potential at the thread's output points now: their
+            // latency passes under the barrier and the shared-memory loads of the last inverse stage
+#pragma unroll
+            for (int it = 0; it < NITEM; ++it)
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const long long gi = (long long)row * N + lt + it * TPL + j * S1;
+                    pold[it][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
+                    vpot[it][j] = __ldg(&a.V[gi]);
+                }
+            if (R2 > 0) group_sync<GT>(g);
         }
         // last inverse stage + crop + window + accumulate + V.u + first forward stage; a thread
-        // writes the slots it has just read, so the items need no barrier between them
-#pragma unroll 1
-        for (int t = lt; t < S1; t += TPL) {
+        // writes the slots it has just read, so the items need no barrier between them.  The p and V
+        // values of all items of the thread were requested before the barrier in front of this stage.
+#pragma unroll
+        for (int it = 0; it < NITEM; ++it) {
+            const int t = lt + it * TPL;
             float2 x[R1];
+            float2 wre[R1], wim[R1];
+            load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
             if (!FIRST) {
-                plast_inv<N, R1, Lay>(x, l, t, wk, a.lut.AB);
+                plast_inv_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
 #pragma unroll
                 for (int j = 0; j < R1; ++j) {
                     const int pos = t + j * S1;
                     const long long gi = (long long)row * N + pos;
                     const float wgt = wrow * __ldg(&a.ax[pos]);
-                    float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
-                    float2 pv = u;
-                    if (term > 0) pv = cadd(a.p[gi], u);
+                    const float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
+                    const float2 pv = cadd(pold[it][j], u);
                     a.p[gi] = pv;
                     uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
                     pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
-                    x[j] = cmul(__ldg(&a.V[gi]), u);
+                    x[j] = cmul(vpot[it][j], u);
                 }
                 if (!a.do_fwd) continue;
             } else {
@@ -302,7 +316,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     x[j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
                 }
             }
-            pfirst_fwd<N, R1, Lay>(x, l, t, wk, a.lut.AB);
+            pfirst_fwd_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
         }
         group_sync<GT>(g);
         if (!FIRST && !a.do_fwd) continue;
