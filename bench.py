@@ -31,8 +31,8 @@ import tbs_workloads as W  # noqa: E402
 
 METRIC = "born_series_grid_point_terms_per_sec"
 UNIT = "grid-point-terms/s"
-ALG_BYTES = {2: {"k_row": 56.0, "k_col_conv": 32.0},
-             3: {"k_row": 56.0, "k_col_fwd_y": 48.0, "k_col_conv_z": 64.0, "k_col_inv_y": 48.0}}
+ALG_BYTES = {2: {"k_row": 56.0, "k_conv": 32.0},
+             3: {"k_row": 56.0, "k_col_fwd_y": 48.0, "k_conv_z": 64.0, "k_col_inv_y": 48.0}}
 
 
 def make_workload(name):

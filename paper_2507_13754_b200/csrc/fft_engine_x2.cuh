@@ -125,17 +125,6 @@ __device__ __forceinline__ void pstage_item(float4 *sm, const float2 *__restrict
     if (S > 1) load_tw<R, S, 1>(tw, lut, b % S);
     pstage_item_tw<N, LB, R, FWD, Lay>(sm, tw, line, b);
 }
-// The same with the twiddles of the thread's first item already in registers (fetched before the
-// barrier that precedes the stage, so that their L2 latency is not exposed after it).
-template <int N, int LB, int R, bool FWD, class Lay, int TPL>
-__device__ __forceinline__ void pstage_line_pre(float4 *sm, const float2 *__restrict__ lut, float2 (&tw)[R], int line, int lt) {
-    constexpr int S = LB / R, NBL = N / R;
-#pragma unroll 1
-    for (int b = lt; b < NBL; b += TPL) {
-        if (b != lt && S > 1) load_tw<R, S, 1>(tw, lut, b % S);
-        pstage_item_tw<N, LB, R, FWD, Lay>(sm, tw, line, b);
-    }
-}
 template <int N, int LB, int R, bool FWD, class Lay, int TPL>
 __device__ __forceinline__ void pstage_line(float4 *sm, const float2 *__restrict__ lut, int line, int lt) {
     constexpr int NBL = N / R;
@@ -210,20 +199,25 @@ __device__ __forceinline__ void plast_inv(float2 (&z)[R1], int line, int t, cons
     plast_inv_tw<N, R1, Lay>(z, line, t, sm, wre, wim);
 }
 
-// Fused middle of the convolution (packed form of mid_conv_item): last forward stage (contiguous
-// blocks of RL), multiply by ghat, first inverse stage, in registers.
-//   k0^2 ghat = (a + i e)/(a^2 + e^2),  a = a_line + p2[half][P],  e = eps/k0^2
-// p2x2: the line-axis table interleaved over the halves, [j][block] float2 = (even, odd).
+// Fused middle of the convolution: last forward stage (contiguous blocks of RL), multiply by ghat,
+// first inverse stage, in registers (north_star: "pointwise G multiply fused into the last forward
+// and first inverse butterfly stage").  With e = eps/k0^2 and alpha = (|p|^2/k0^2 - 1)/e,
+//   k0^2 ghat = 1/(e (alpha - i)) = (alpha + i) / (e (alpha^2 + 1))
+// so v ghat = ((v.re alpha - v.im) + i (v.im alpha + v.re)) / (alpha^2 + 1): six packed operations
+// and one MUFU.RCP per half; the constant 1/(e k0^2) rides on the normalisation applied by k_row.
+// p2x2: the line-axis table |p|^2/(e k0^2), interleaved over the halves, [j][block] float2 = (even, odd);
+// a_line: (|p|^2 of the other axes / k0^2 - 1) / e.
 template <int N, int RL>
 __device__ __forceinline__ void load_p2x2(float2 (&pp)[RL], const float2 *__restrict__ p2x2, int b) {
 #pragma unroll
     for (int j = 0; j < RL; ++j) pp[j] = __ldg(p2x2 + j * (N / RL) + b);
 }
 template <int N, int RL, class Lay>
-__device__ __forceinline__ void pmid_conv_item_pp(float4 *sm, int line, int b, const float2 (&pp)[RL],
-                                                  float a_line, float e) {
+__device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
+                                               float a_line) {
     const int base = b * RL;
-    const float e2 = e * e;
+    float2 pp[RL];
+    load_p2x2<N, RL>(pp, p2x2, b);
     P2 v[RL];
 #pragma unroll
     for (int j = 0; j < RL; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j));
@@ -232,22 +226,14 @@ __device__ __forceinline__ void pmid_conv_item_pp(float4 *sm, int line, int b, c
 #pragma unroll
     for (int i = 0; i < RL; ++i) {
         const int k = brev(i, RL);
-        const float2 a = __fadd2_rn(pp[k], f2(a_line));
-        const float2 d = __ffma2_rn(a, a, f2(e2));
+        const float2 al = __fadd2_rn(pp[k], f2(a_line));
+        const float2 d = __ffma2_rn(al, al, f2(1.0f));
         const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
-        const float2 tx = __fmul2_rn(v[i].re, r), ty = __fmul2_rn(v[i].im, r);
-        u[k] = P2{__ffma2_rn(tx, a, __fmul2_rn(ty, f2(-e))), __ffma2_rn(tx, f2(e), __fmul2_rn(ty, a))};
+        u[k] = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};
     }
     pbfly<RL, +1>(u);
 #pragma unroll
     for (int i = 0; i < RL; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, RL)), u[i]);
-}
-template <int N, int RL, class Lay>
-__device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
-                                               float a_line, float e) {
-    float2 pp[RL];
-    load_p2x2<N, RL>(pp, p2x2, b);
-    pmid_conv_item_pp<N, RL, Lay>(sm, line, b, pp, a_line, e);
 }
 
 }  // namespace tbs

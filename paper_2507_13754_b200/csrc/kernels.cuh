@@ -36,10 +36,10 @@ struct ColArgs {
     long long in_outer_stride, out_outer_stride;  // between consecutive outer indices
     int inner_len;                                // number of adjacent lines (multiple of T)
     int n_outer;                                  // number of outer indices
-    const float2 *p2_line;  // [N] (even, odd) |p|^2/k0^2 of the line axis, order of pmid_conv_item
+    const float2 *p2_line;  // [N] (even, odd) |p|^2/eps of the line axis, order of pmid_conv_item
     const float *p2_inner;  // [inner_len] of the inner (x) axis, position order  (CONV)
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
-    float e;                // eps/k0^2                                           (CONV)
+    float inv_e;            // k0^2/eps = 1/damping
     Luts lut;
     const Ctl *ctl;
 };
@@ -166,7 +166,7 @@ struct RowArgs {
     int ny;               // rows = ny * nz; row = z*ny + y
     int rows;
     float src_scale;      // FIRST: 1/k0^2
-    float scale;          // 1/prod(2 n): normalisation of the inverse transforms of all axes
+    float scale;          // k0^2/(eps prod(2 n)): inverse-transform normalisation and the 1/e of ghat (k_conv)
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
@@ -459,8 +459,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
         {
             float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
             if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
+            a_line *= a.inv_e;
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line, a.e);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line);
             if (more) stage_part(tile + gridDim.x, 1);
             group_sync<GT>(g);
         }

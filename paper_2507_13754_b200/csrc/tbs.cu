@@ -102,7 +102,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.ny = pl->n[1];
     a.rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
     a.src_scale = src_scale;
-    a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0));
+    a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
     a.do_fwd = do_fwd;
     a.norms = pl->norms;
     a.history = pl->history;
@@ -117,7 +117,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     ColArgs a;
     memset(&a, 0, sizeof a);
     a.ctl = f.ctl;
-    a.e = (float)pl->damping;
+    a.inv_e = (float)(1.0 / pl->damping);
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
@@ -305,7 +305,7 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
                 radices_of(pl->n[a], r1, r2, rl);
                 CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
                 k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, dx_m, f.k0,
-                                                                 a == 0 || a == ndim - 1);
+                                                                 a == 0 || a == ndim - 1, a == ndim - 1 ? 1.0 / damping : 1.0);
             }
         }
         CU(pl, cudaDeviceSynchronize());
