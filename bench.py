@@ -33,6 +33,17 @@ METRIC = "born_series_grid_point_terms_per_sec"
 UNIT = "grid-point-terms/s"
 ALG_BYTES = {2: {"k_row": 56.0, "k_conv": 32.0},
              3: {"k_row": 56.0, "k_col_fwd_y": 48.0, "k_conv_z": 64.0, "k_col_inv_y": 48.0}}
+# From the committed ncu captures (profiles/r01b_ncu_summary.md), per launch of the named workload:
+#   traffic  = dram__bytes_read.sum + dram__bytes_write.sum
+#   fp32_res = FP32 results issued (packed instructions count twice), from smsp__inst_executed x mix
+NCU = {
+    "cfg3": {"k_conv": {"traffic": 67.22e6 + 26.15e6, "fp32_res": 42.12e6 * 32 * (2 * 0.464 + 0.036)},
+             "k_row": {"traffic": 134.32e6 + 44.94e6, "fp32_res": 19.58e6 * 32 * (2 * 0.466 + 0.139)}},
+    "cfg5": {"k_conv_z": {"traffic": 537.10e6 + 483.35e6, "fp32_res": 234.48e6 * 32 * (2 * 0.478 + 0.080)},
+             "k_col_fwd_y": {"traffic": 268.46e6 + 481.47e6, "fp32_res": 80.53e6 * 32 * 0.672},
+             "k_row": {"traffic": 537.10e6 + 347.03e6, "fp32_res": 58.50e6 * 32 * (2 * 0.435 + 0.197)}},
+}
+FP32_PEAK = 148 * 128 * 1.965e9   # FP32 results/s: 128 lanes/clk/SM (packed f32x2 counts as 2 results, same pipe)
 
 
 def make_workload(name):
@@ -256,6 +267,12 @@ def main():
         b = ALG_BYTES[w.ndim][name] * w.n_points
         kernels.append({"kernel": name, "ms": float(ms), "alg_bytes": b, "achieved_gbs": b / (ms * 1e-3) / 1e9,
                         "frac": b / (ms * 1e-3) / 1e9 / peak})
+    ncu = NCU.get(args.workload, {})
+    for k in kernels:
+        c = ncu.get(k["kernel"])
+        if c:
+            k["dram_traffic_ncu"] = c["traffic"]
+            k["fp32_frac"] = c["fp32_res"] / (k["ms"] * 1e-3) / FP32_PEAK
     dom = max(kernels, key=lambda k: k["ms"])
     term_ms = loop_ms / max(local_terms, 1)
     term_bytes = sum(ALG_BYTES[w.ndim].values()) * w.n_points
@@ -277,7 +294,9 @@ def main():
                 "ms_per_step": 1e3 * e2e_s / args.steps},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
-                     "unit": "GB/s", "frac": dom["frac"], "traffic": None, "peak_source": peak_src},
+                     "unit": "GB/s", "frac": dom["frac"], "traffic": dom.get("dram_traffic_ncu"),
+                     "traffic_source": "profiles/r01b_ncu_summary.md (ncu --set full, same workload)",
+                     "peak_source": peak_src, "fp32_pipe_frac": dom.get("fp32_frac")},
         "kernels": kernels,
         "term_loop": {"ms_per_term": term_ms, "alg_bytes_per_term": term_bytes,
                       "achieved_gbs": term_bytes / (term_ms * 1e-3) / 1e9,
