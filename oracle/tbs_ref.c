@@ -341,3 +341,29 @@ int tbs_ref_second_harmonic_source(int64_t n, const double *p1_reim, double beta
     for (int64_t i = 0; i < n; ++i) S2[i] = -xi * w2 * w2 * 0.5 * p1[i] * p1[i];
     return TBS_REF_OK;
 }
+
+/* ---- Harmonic sources 2..5, Eqs. 28b-28e (sum-frequency terms only, the
+ * difference terms are dropped); xi of PAPER.md:117.
+ *   S_h(r) = -xi (h omega1)^2 C_h(r),
+ *   C_2 = psi1^2/2, C_3 = psi1 psi2, C_4 = psi2^2/2 + psi1 psi3, C_5 = psi2 psi3 + psi1 psi4.
+ * psi_reim[m] is the field of harmonic m+1 (only those below h are read). */
+int tbs_ref_harmonic_source(int64_t n, int h, const double *const *psi_reim, double beta, double rho0,
+                            double c0, double f1_hz, double *S_reim) {
+    if (n <= 0 || h < 2 || h > 5 || rho0 <= 0 || c0 <= 0) return TBS_REF_ERR_INVALID_ARG;
+    const cplx *p1 = (const cplx *)psi_reim[0];
+    const cplx *p2 = h >= 3 ? (const cplx *)psi_reim[1] : NULL;
+    const cplx *p3 = h >= 4 ? (const cplx *)psi_reim[2] : NULL;
+    const cplx *p4 = h >= 5 ? (const cplx *)psi_reim[3] : NULL;
+    cplx *S = (cplx *)S_reim;
+    double xi = beta / (rho0 * c0 * c0 * c0 * c0);
+    double wh = (double)h * (2.0 * PI * f1_hz);
+    for (int64_t i = 0; i < n; ++i) {
+        cplx C;
+        if (h == 2) C = 0.5 * p1[i] * p1[i];
+        else if (h == 3) C = p1[i] * p2[i];
+        else if (h == 4) C = 0.5 * p2[i] * p2[i] + p1[i] * p3[i];
+        else C = p2[i] * p3[i] + p1[i] * p4[i];
+        S[i] = -xi * wh * wh * C;
+    }
+    return TBS_REF_OK;
+}

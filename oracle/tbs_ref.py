@@ -53,6 +53,8 @@ def lib() -> ctypes.CDLL:
         L.tbs_ref_second_harmonic_source.argtypes = [ctypes.c_int64, dp, ctypes.c_double,
                                                      ctypes.c_double, ctypes.c_double,
                                                      ctypes.c_double, dp]
+        L.tbs_ref_harmonic_source.argtypes = [ctypes.c_int64, ctypes.c_int, ctypes.POINTER(dp), ctypes.c_double,
+                                              ctypes.c_double, ctypes.c_double, ctypes.c_double, dp]
         _lib = L
     return _lib
 
@@ -186,3 +188,15 @@ def second_harmonic_source(p1, beta: float, rho0: float, c0: float, f1_hz: float
     rc = lib().tbs_ref_second_harmonic_source(p1.size, _dp(p1), beta, rho0, c0, f1_hz, _dp(S2))
     assert rc == OK, rc
     return S2
+
+
+def harmonic_source(h: int, fields, beta: float, rho0: float, c0: float, f1_hz: float):
+    """S_h of Eqs. 28b-28e from the fields of harmonics 1..h-1 (`fields[m]` = psi_{m+1})."""
+    fs = [np.ascontiguousarray(f, dtype=np.complex128) for f in fields[:h - 1]]
+    assert len(fs) == h - 1
+    S = np.empty_like(fs[0])
+    dp = ctypes.POINTER(ctypes.c_double)
+    ptrs = (dp * 4)(*([_dp(f) for f in fs] + [None] * (4 - len(fs))))
+    rc = lib().tbs_ref_harmonic_source(fs[0].size, int(h), ptrs, beta, rho0, c0, f1_hz, _dp(S))
+    assert rc == OK, rc
+    return S

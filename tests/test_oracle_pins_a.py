@@ -172,3 +172,30 @@ def test_second_harmonic_source_is_2w_component_of_westervelt(golden):
         comp = 2 * np.mean(xi * d2 * np.exp(2j * w * t))
         # equation: lap psi2 + k2^2 psi2 + comp = 0  ->  rhs = -comp = -S2
         assert abs(S2[i] - comp) < 2e-5 * abs(comp)
+
+
+@pytest.mark.parametrize("h", [2, 3, 4, 5])
+def test_harmonic_sources_are_sum_frequency_components_of_westervelt(golden, h):
+    """Eqs. 27b-27e / 28b-28e: with Psi = Re(Psi+), Psi+ = sum_m psi_m e^{-i m w t},
+    Psi^2 = (Psi+^2 + Psi+*^2)/4 + |Psi+|^2/2; the paper keeps the sum-frequency part Re(Psi+^2)/2 and
+    drops the difference terms.  S_h is minus the e^{-i h w t} component of
+    xi d^2/dt^2 of that part -- evaluated here by a numerical time derivative and projection."""
+    f = golden["f_hz"]
+    w = 2 * math.pi * f
+    beta = 1 + golden["b_over_a"] / 2
+    rho, c = golden["rho_f"], golden["v_f"]
+    xi = beta / (rho * c ** 4)
+    rng = np.random.default_rng(5)
+    psi = [(rng.standard_normal(3) + 1j * rng.standard_normal(3)) * s for s in (1e5, 3e4, 1e4, 3e3)]
+    S = R.harmonic_source(h, psi, beta, rho, c, f)
+    nt = 8192
+    t = np.arange(nt) / nt * (2 * math.pi / w)
+    dt = t[1] - t[0]
+    for i in range(3):
+        plus = sum(psi[m][i] * np.exp(-1j * (m + 1) * w * t) for m in range(h - 1))
+        X = (plus ** 2).real / 2
+        d2 = (np.roll(X, -1) - 2 * X + np.roll(X, 1)) / dt ** 2
+        comp = 2 * np.mean(xi * d2 * np.exp(1j * h * w * t))
+        assert abs(S[i] - comp) < 1e-4 * abs(comp)
+    if h == 2:
+        assert np.allclose(S, R.second_harmonic_source(psi[0], beta, rho, c, f), rtol=1e-14)
