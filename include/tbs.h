@@ -115,6 +115,18 @@ tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, 
                                      float *p2_out, double *history1, double *history2,
                                      int32_t *n_terms1, int32_t *n_terms2, void *stream);
 
+/* Harmonics 1..n_harm (n_harm <= 5) of a nonlinear medium, one after the other (Eqs. 27-28,
+ * PAPER.md:266): plans[h-1] is a plan with nfreq = 1 created at h*f1 on the same grid with its medium set
+ * (so k0 -> h k0, eps_h = damping (h k0)^2, absorption at h w).  The fundamental is solved from its own
+ * source, optionally rescaled as in tbs_solve_second_harmonic, and harmonic h >= 2 from
+ *   S_h = -xi (h w1)^2 C_h,  C_2 = psi1^2/2, C_3 = psi1 psi2, C_4 = psi2^2/2 + psi1 psi3,
+ *   C_5 = psi2 psi3 + psi1 psi4   (sum-frequency terms only), xi = beta/(rho0 c0^4) of plans[0].
+ * p_out[h-1] dev [n][2]; history[h-1] host [max_terms+1]; n_terms host [n_harm].  Host arrays of pointers.
+ * Returns the worst status; a negative status of one harmonic stops the chain. */
+tbs_status tbs_solve_harmonics(tbs_plan *const *plans, int n_harm, int max_terms, double tol, int ref_row,
+                               double surface_pressure_pa, float *const *p_out, double *const *history,
+                               int32_t *n_terms, void *stream);
+
 /* Introspection for tests and the bench. */
 /* One application of G to x (dev [n][2]) for frequency ifreq: out = crop IDFT ghat DFT pad x. */
 tbs_status tbs_apply_green(tbs_plan *plan, int ifreq, const float *x, float *out, void *stream);

@@ -166,17 +166,30 @@ __global__ void k_row_max(const float2 *p, long long first, long long count, uns
     if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));
 }
 
-// p1 <- g p1 (g = target / max|p1| when target > 0), S2 = -xi (2 w1)^2 (1/2) p1^2
-// (Eq. 28b; xi = beta/(rho0 c0^4)).
-__global__ void k_second_harmonic_source(float2 *p1, float2 *S2, const unsigned int *max2bits,
-                                         double target, double coef, long long n) {
+// p1 <- g p1 with g = target / max|p1| over the reference row ("surface pressure", reading A10).
+__global__ void k_rescale_field(float2 *p1, const unsigned int *max2bits, double target, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    double g = 1.0;
-    if (target > 0.0) g = target / sqrt((double)__uint_as_float(*max2bits));
-    const double re = (double)p1[i].x * g, im = (double)p1[i].y * g;
-    p1[i] = make_float2((float)re, (float)im);
-    S2[i] = make_float2((float)(coef * (re * re - im * im)), (float)(coef * 2.0 * re * im));
+    const double g = target / sqrt((double)__uint_as_float(*max2bits));
+    p1[i] = make_float2((float)((double)p1[i].x * g), (float)((double)p1[i].y * g));
+}
+
+// Harmonic source (Eqs. 28b-28e; xi = beta/(rho0 c0^4)):
+//   S = coef (wab pa pb + wcd pc pd),  coef = -xi (h w1)^2;
+//   h = 2: pa = pb = psi1, wab = 1/2;   h = 3: psi1 psi2;
+//   h = 4: psi2 psi2 / 2 + psi1 psi3;   h = 5: psi2 psi3 + psi1 psi4   (pc = nullptr: one product).
+__global__ void k_harmonic_source(float2 *S, double coef, const float2 *pa, const float2 *pb, double wab,
+                                  const float2 *pc, const float2 *pd, double wcd, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double ar = pa[i].x, ai = pa[i].y, br = pb[i].x, bi = pb[i].y;
+    double re = wab * (ar * br - ai * bi), im = wab * (ar * bi + ai * br);
+    if (pc) {
+        const double cr = pc[i].x, ci = pc[i].y, dr = pd[i].x, di = pd[i].y;
+        re += wcd * (cr * dr - ci * di);
+        im += wcd * (cr * di + ci * dr);
+    }
+    S[i] = make_float2((float)(coef * re), (float)(coef * im));
 }
 
 }  // namespace tbs

@@ -152,35 +152,75 @@ tbs_status tbs_apply_green(tbs_plan *pl, int ifreq, const float *x, float *out, 
     return TBS_OK;
 }
 
+tbs_status tbs_solve_harmonics(tbs_plan *const *plans, int n_harm, int max_terms, double tol, int ref_row,
+                               double surface_pressure_pa, float *const *p_out, double *const *history,
+                               int32_t *n_terms, void *stream) {
+    if (!plans || n_harm < 1 || n_harm > 5 || !p_out || !history || !n_terms) return TBS_ERR_INVALID_ARG;
+    for (int h = 0; h < n_harm; ++h)
+        if (!plans[h] || !p_out[h] || !history[h] || plans[h]->fr.size() != 1) return TBS_ERR_INVALID_ARG;
+    tbs_plan *p1 = plans[0];
+    for (int h = 1; h < n_harm; ++h) {
+        tbs_plan *ph = plans[h];
+        if (ph->ndim != p1->ndim) return fail(ph, TBS_ERR_INVALID_ARG, "plans differ in dimension");
+        for (int a = 0; a < 3; ++a)
+            if (p1->n[a] != ph->n[a]) return fail(ph, TBS_ERR_INVALID_ARG, "plans differ in grid size");
+        if (fabs(ph->fr[0].f - (h + 1) * p1->fr[0].f) > 1e-9 * p1->fr[0].f)
+            return fail(ph, TBS_ERR_INVALID_ARG, "plan %d must be created at %d times the fundamental", h, h + 1);
+    }
+    const int nslow = p1->ndim == 2 ? p1->n[1] : p1->n[2];
+    if (ref_row < 0 || ref_row >= nslow) return fail(p1, TBS_ERR_INVALID_ARG, "ref_row outside the grid");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long n = p1->npts;
+    tbs_status res = solve_all(p1, max_terms, tol, p_out[0], false, history[0], &n_terms[0], st);
+    if (res < 0) return res;
+    if (surface_pressure_pa > 0.0) {
+        const long long slab = n / nslow;
+        cudaMemsetAsync(p1->maxbits, 0, sizeof(unsigned int), st);
+        k_row_max<<<nblk(slab, 256), 256, 0, st>>>(p1->fr[0].p, (long long)ref_row * slab, slab, p1->maxbits);
+        k_rescale_field<<<nblk(n, 256), 256, 0, st>>>(p1->fr[0].p, p1->maxbits, surface_pressure_pa, n);
+        CU(p1, cudaGetLastError());
+        CU(p1, cudaMemcpyAsync(p_out[0], p1->fr[0].p, sizeof(float2) * n, cudaMemcpyDeviceToDevice, st));
+        p1->launches += 2;
+    }
+    // xi = beta/(rho0 c0^4); S_h = -xi (h w1)^2 C_h (Eqs. 28b-28e)
+    const double xi = p1->beta / (p1->rho0 * pow(p1->c0, 4.0));
+    for (int h = 2; h <= n_harm; ++h) {
+        tbs_plan *ph = plans[h - 1];
+        const double wh = (double)h * p1->fr[0].omega;
+        const double coef = -xi * wh * wh;
+        const float2 *f1 = plans[0]->fr[0].p;
+        const float2 *f2 = h >= 3 ? plans[1]->fr[0].p : nullptr;
+        const float2 *f3 = h >= 4 ? plans[2]->fr[0].p : nullptr;
+        const float2 *f4 = h >= 5 ? plans[3]->fr[0].p : nullptr;
+        float2 *S = ph->fr[0].S;
+        const unsigned g = nblk(n, 256);
+        if (h == 2) k_harmonic_source<<<g, 256, 0, st>>>(S, coef, f1, f1, 0.5, nullptr, nullptr, 0.0, n);
+        else if (h == 3) k_harmonic_source<<<g, 256, 0, st>>>(S, coef, f1, f2, 1.0, nullptr, nullptr, 0.0, n);
+        else if (h == 4) k_harmonic_source<<<g, 256, 0, st>>>(S, coef, f2, f2, 0.5, f1, f3, 1.0, n);
+        else k_harmonic_source<<<g, 256, 0, st>>>(S, coef, f2, f3, 1.0, f1, f4, 1.0, n);
+        CU(ph, cudaGetLastError());
+        ph->fr[0].have_S = true;
+        tbs_status sh = solve_all(ph, max_terms, tol, p_out[h - 1], false, history[h - 1], &n_terms[h - 1], st);
+        ph->launches += 1;
+        if (sh < 0) return sh;
+        res = worst(res, sh);
+    }
+    return res;
+}
+
 tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, double tol, int ref_row,
                                      double surface_pressure_pa, float *p1_out, float *p2_out,
                                      double *history1, double *history2, int32_t *n_terms1,
                                      int32_t *n_terms2, void *stream) {
-    if (!p1 || !p2 || p1->fr.size() != 1 || p2->fr.size() != 1 || p1->ndim != p2->ndim) return TBS_ERR_INVALID_ARG;
-    for (int a = 0; a < 3; ++a)
-        if (p1->n[a] != p2->n[a]) return fail(p2, TBS_ERR_INVALID_ARG, "plans differ in grid size");
-    if (fabs(p2->fr[0].f - 2.0 * p1->fr[0].f) > 1e-9 * p1->fr[0].f)
-        return fail(p2, TBS_ERR_INVALID_ARG, "second plan must be created at twice the fundamental");
-    const int nslow = p1->ndim == 2 ? p1->n[1] : p1->n[2];
-    if (ref_row < 0 || ref_row >= nslow) return fail(p1, TBS_ERR_INVALID_ARG, "ref_row outside the grid");
-    cudaStream_t st = (cudaStream_t)stream;
-    tbs_status s1 = solve_all(p1, max_terms, tol, p1_out, false, history1, n_terms1, st);
-    if (s1 < 0) return s1;
-    // S2 = -xi (2 w1)^2 (1/2) p1^2, xi = beta/(rho0 c0^4)  (Eq. 28b)
-    const double xi = p1->beta / (p1->rho0 * pow(p1->c0, 4.0));
-    const double w2 = 2.0 * p1->fr[0].omega;
-    const double coef = -xi * w2 * w2 * 0.5;
-    const long long slab = p1->npts / nslow;
-    cudaMemsetAsync(p1->maxbits, 0, sizeof(unsigned int), st);
-    k_row_max<<<nblk(slab, 256), 256, 0, st>>>(p1->fr[0].p, (long long)ref_row * slab, slab, p1->maxbits);
-    k_second_harmonic_source<<<nblk(p1->npts, 256), 256, 0, st>>>(p1->fr[0].p, p2->fr[0].S, p1->maxbits,
-                                                                   surface_pressure_pa, coef, p1->npts);
-    CU(p1, cudaGetLastError());
-    CU(p1, cudaMemcpyAsync(p1_out, p1->fr[0].p, sizeof(float2) * p1->npts, cudaMemcpyDeviceToDevice, st));
-    p2->fr[0].have_S = true;
-    tbs_status s2 = solve_all(p2, max_terms, tol, p2_out, false, history2, n_terms2, st);
-    p1->launches += 2;
-    return worst(s1, s2);
+    if (!n_terms1 || !n_terms2) return TBS_ERR_INVALID_ARG;
+    tbs_plan *plans[2] = {p1, p2};
+    float *outs[2] = {p1_out, p2_out};
+    double *hist[2] = {history1, history2};
+    int32_t nt[2] = {0, 0};
+    const tbs_status s = tbs_solve_harmonics(plans, 2, max_terms, tol, ref_row, surface_pressure_pa, outs, hist, nt, stream);
+    *n_terms1 = nt[0];
+    *n_terms2 = nt[1];
+    return s;
 }
 
 tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4], void *stream) {

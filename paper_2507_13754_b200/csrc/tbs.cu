@@ -128,7 +128,6 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         if (which < 0 || which == 0) e = launch_conv(ny, a, 1, st);
         return e;
     }
-    const long long mz = 2LL * nz;
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
     if (which < 0 || which == 0) {
         a.in = pl->W1; a.out = pl->W2;

@@ -212,3 +212,24 @@ def solve_second_harmonic(plan1: Plan, plan2: Plan, max_terms, tol, ref_row, sur
     r1 = SolveResult(st, p1, h1, n1, plan1.last_loop_ms(), plan1.last_launch_count())
     r2 = SolveResult(st, p2, h2, n2, plan2.last_loop_ms(), plan2.last_launch_count())
     return st, (r1, r2)
+
+
+def solve_harmonics(plans, max_terms, tol, ref_row, surface_pressure_pa):
+    """tbs_solve_harmonics: plans[h-1] created at h*f1; returns (status, [SolveResult per harmonic])."""
+    L = plans[0]._L
+    nh = len(plans)
+    vp, dp, ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)
+    outs = [torch.empty((1,) + pl.shape, dtype=torch.complex64, device="cuda") for pl in plans]
+    hists = [np.zeros((1, max_terms + 1), dtype=np.float64) for _ in plans]
+    nt = np.zeros(nh, dtype=np.int32)
+    h_arr = (vp * nh)(*[pl._h for pl in plans])
+    o_arr = (vp * nh)(*[vp(o.data_ptr()) for o in outs])
+    hi_arr = (dp * nh)(*[h.ctypes.data_as(dp) for h in hists])
+    st = L.tbs_solve_harmonics(h_arr, nh, int(max_terms), float(tol), int(ref_row), float(surface_pressure_pa),
+                               o_arr, hi_arr, nt.ctypes.data_as(ip), _stream_ptr())
+    if st not in (OK, NOT_CONVERGED, ERR_DIVERGED):
+        msgs = [L.tbs_last_error(pl._h).decode() for pl in plans]
+        raise TbsError(st, next((m for m in msgs if m), ""))
+    res = [SolveResult(st, outs[i], hists[i], nt[i:i + 1].copy(), plans[i].last_loop_ms(), plans[i].last_launch_count())
+           for i in range(nh)]
+    return st, res
