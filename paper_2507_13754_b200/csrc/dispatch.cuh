@@ -59,12 +59,48 @@ static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, 
     return cudaGetLastError();
 }
 
+#ifndef TBS_CONV_TMA
+#define TBS_CONV_TMA 1   // 1: input tiles through the tensor map (TMA); 0: 16-byte cp.async copies
+#endif
+
+// Tensor map of the array k_conv reads: a 2-D tensor of 8-byte elements, dim0 = all columns (x, or
+// (ky, kx) in the 3-D z pass), dim1 = the N positions along the line; box = T columns x min(N, 256) rows,
+// hardware swizzle matched to the 16-byte-chunk XOR of the staging layout.
+typedef CUresult (*tbs_encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                        const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                        CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                        CUtensorMapFloatOOBfill);
+static inline cudaError_t make_conv_tensor_map(CUtensorMap *out, const void *base, long long n_cols, int n_rows,
+                                               long long row_stride_elems, int T) {
+    static tbs_encode_tiled_fn enc = nullptr;
+    if (!enc) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+        if (e != cudaSuccess) return e;
+        if (q != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+        enc = (tbs_encode_tiled_fn)fn;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)n_cols, (cuuint64_t)n_rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)row_stride_elems * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)T, (cuuint32_t)(n_rows < 256 ? n_rows : 256)};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUtensorMapSwizzle sw = T >= 16 ? CU_TENSOR_MAP_SWIZZLE_128B
+                                 : T == 8 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                 : T == 4 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
+    const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<void *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+static inline int conv_tile_width(int N);
+
 template <int N>
-static cudaError_t launch_conv_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr) {
+static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr) {
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = T * tpl_of(N);
-    constexpr size_t smem = (2 * (size_t)T * LineLay<N, conv_pad(N, T)>::PITCH + (size_t)N * T) * sizeof(float2);
-    auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
+    constexpr size_t smem = (size_t)conv_stage_offset(N, T) + (size_t)N * T * sizeof(float2);
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB, TBS_CONV_TMA != 0>;
     static int cap = 0;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -74,23 +110,31 @@ static cudaError_t launch_conv_t(const ColArgs &a, int n_outer, cudaStream_t st,
     ColArgs b = a;
     b.n_outer = n_outer;
     const long long total = (long long)n_outer * (a.inner_len / T);
-    kern<<<(unsigned)(total < cap ? total : cap), NT, smem, st>>>(b);
+    kern<<<(unsigned)(total < cap ? total : cap), NT, smem, st>>>(b, *tmap);
     return cudaGetLastError();
 }
 
-static cudaError_t launch_conv(int N, const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr = false) {
+static cudaError_t launch_conv(int N, const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st,
+                               bool set_attr = false) {
     switch (N) {
-        case 32:   return launch_conv_t<32>(a, n_outer, st, set_attr);
-        case 64:   return launch_conv_t<64>(a, n_outer, st, set_attr);
-        case 128:  return launch_conv_t<128>(a, n_outer, st, set_attr);
-        case 256:  return launch_conv_t<256>(a, n_outer, st, set_attr);
-        case 512:  return launch_conv_t<512>(a, n_outer, st, set_attr);
-        case 1024: return launch_conv_t<1024>(a, n_outer, st, set_attr);
-        case 2048: return launch_conv_t<2048>(a, n_outer, st, set_attr);
-        case 4096: return launch_conv_t<4096>(a, n_outer, st, set_attr);
+        case 32:   return launch_conv_t<32>(a, tmap, n_outer, st, set_attr);
+        case 64:   return launch_conv_t<64>(a, tmap, n_outer, st, set_attr);
+        case 128:  return launch_conv_t<128>(a, tmap, n_outer, st, set_attr);
+        case 256:  return launch_conv_t<256>(a, tmap, n_outer, st, set_attr);
+        case 512:  return launch_conv_t<512>(a, tmap, n_outer, st, set_attr);
+        case 1024: return launch_conv_t<1024>(a, tmap, n_outer, st, set_attr);
+        case 2048: return launch_conv_t<2048>(a, tmap, n_outer, st, set_attr);
+        case 4096: return launch_conv_t<4096>(a, tmap, n_outer, st, set_attr);
         default: break;
     }
     return cudaErrorInvalidValue;
+}
+static inline int conv_tile_width(int N) {
+    switch (N) {
+        case 32: return ConvCfg<32>::T;     case 64: return ConvCfg<64>::T;     case 128: return ConvCfg<128>::T;
+        case 256: return ConvCfg<256>::T;   case 512: return ConvCfg<512>::T;   case 1024: return ConvCfg<1024>::T;
+        case 2048: return ConvCfg<2048>::T; default: return ConvCfg<4096>::T;
+    }
 }
 
 template <int MODE>

@@ -46,6 +46,11 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
 }
+// 2-D tiled TMA load (cp.async.bulk.tensor): box at element coordinates (c0, c1) of the tensor map.
+__device__ __forceinline__ void tma_load_2d(void *dst, const void *tmap, int c0, int c1, uint64_t *b) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(b)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
     uint32_t ok;
     do {
@@ -198,6 +203,10 @@ struct RowLay {
 // half-warp, 4 line pairs x 4 positions when T >= 8; a pitch of 2 modulo 8 spreads them evenly.
 __host__ __device__ constexpr int conv_pad(int N, int T) {
     return T >= 8 ? (2 + 16 - (N + N / 16) % 8) % 8 : 0;
+}
+// Byte offset of k_conv's staging buffer behind its work area, rounded to the 1024-byte swizzle atom.
+__host__ __device__ constexpr int conv_stage_offset(int N, int T) {
+    return (T * (N + N / 16 + conv_pad(N, T)) * 16 + 1023) / 1024 * 1024;
 }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
 template <int GT>

@@ -12,6 +12,8 @@
 // Both parity halves of a padded line (fft_engine.cuh) are resident in shared memory at once, so
 // the input is read once and the twiddles of a butterfly pair are fetched once.
 #pragma once
+#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime, tbs.cu)
+
 #include "fft_engine_x2.cuh"
 
 namespace tbs {
@@ -384,8 +386,8 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
 // cp.async into a staging buffer while tile i computes; the result goes back through the work area
 // so that global reads and writes are 16 bytes per lane over adjacent lines.  Between the three
 // CTA-wide barriers of a tile the T line groups run on their own barriers.
-template <int N, int T, int MINB>
-__global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
+template <int N, int T, int MINB, bool USE_TMA>
+__global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
@@ -396,12 +398,13 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
     using Lay = LineLay<N, conv_pad(N, T)>;
-    extern __shared__ __align__(128) float2 sm[];
+    extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
     // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
     // 2c+1), the chunk index XOR-swizzled with the position so that the cp.async writes of a warp are
     // contiguous and the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
-    float4 *stg = wk + T * Lay::PITCH;
+    float4 *stg = wk + conv_stage_offset(N, T) / 16;  // 1024-byte aligned (TMA swizzle atom)
+    __shared__ __align__(8) uint64_t mbar;
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
@@ -428,7 +431,22 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
         for (int q = 0; q < NQ; ++q) stage_part(tile, q);
         cp_async_commit();
     };
-    if ((int)blockIdx.x < total) stage_tile(blockIdx.x);
+    // USE_TMA: the same tile arrives as N/BR boxes of BR rows x T columns through the tensor map
+    // (cp.async.bulk.tensor, hardware swizzle = the XOR above), issued by one thread, completion on mbar.
+    constexpr int BR = N < 256 ? N : 256;
+    constexpr uint32_t TILE_BYTES = (uint32_t)N * T * sizeof(float2);
+    uint32_t phase = 0;
+    auto tma_tile = [&](int tile) {
+        mbar_expect_tx(&mbar, TILE_BYTES);
+        const int c0 = (tile / tiles) * (int)a.in_outer_stride + (tile % tiles) * T;
+#pragma unroll 1
+        for (int k = 0; k < N / BR; ++k) tma_load_2d(stg + k * BR * CPR, &tmap, c0, k * BR, &mbar);
+    };
+    if (USE_TMA) {
+        if (tid == 0) mbar_init(&mbar, 1);
+        __syncthreads();
+        if (tid == 0 && (int)blockIdx.x < total) tma_tile(blockIdx.x);
+    } else if ((int)blockIdx.x < total) stage_tile(blockIdx.x);
     const float2 *stg2 = reinterpret_cast<const float2 *>(stg) + (line & 1);
 
 #pragma unroll 1
@@ -436,7 +454,12 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
         const int inner0 = (tile % tiles) * T;
         const int outer = tile / tiles;
         const bool more = tile + (int)gridDim.x < total;
-        cp_async_wait_all();
+        if (USE_TMA) {
+            mbar_wait(&mbar, phase);
+            phase ^= 1u;
+        } else {
+            cp_async_wait_all();
+        }
         __syncthreads();  // staged tile visible; the copy-out of the previous tile has left the work area
         // ---- forward: N inputs -> both halves ----
 #pragma unroll 1
@@ -451,7 +474,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
         }
         __syncthreads();  // staging buffer free (and the line groups are in step)
         // the cp.async copies of the next tile are issued in four parts, one after each stage
-        if (more) stage_part(tile + gridDim.x, 0);
+        if (USE_TMA) {
+            if (more && tid == 0) tma_tile(tile + gridDim.x);
+        } else if (more) stage_part(tile + gridDim.x, 0);
         if (R2 > 0) {
             pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, line, lt);
             group_sync<GT>(g);
@@ -462,15 +487,15 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
             a_line *= a.inv_e;
 #pragma unroll 1
             for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line);
-            if (more) stage_part(tile + gridDim.x, 1);
+            if (!USE_TMA && more) stage_part(tile + gridDim.x, 1);
             group_sync<GT>(g);
         }
         // ---- inverse: both halves -> N outputs, left in the first 8 bytes of their slots ----
         if (R2 > 0) {
             pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, line, lt);
-            if (more) stage_part(tile + gridDim.x, 2);
+            if (!USE_TMA && more) stage_part(tile + gridDim.x, 2);
             group_sync<GT>(g);
-        } else if (more) {
+        } else if (!USE_TMA && more) {
             stage_part(tile + gridDim.x, 2);
         }
 #pragma unroll 1
@@ -480,7 +505,7 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a) {
 #pragma unroll
             for (int j = 0; j < R1; ++j) *reinterpret_cast<float2 *>(wk + Lay::addr(line, t + j * S1)) = z[j];
         }
-        if (more) {
+        if (!USE_TMA && more) {
             stage_part(tile + gridDim.x, 3);
             cp_async_commit();
         }

@@ -45,6 +45,7 @@ struct tbs_plan {
     float4 *lutAB[3] = {nullptr, nullptr, nullptr};
     float2 *W1 = nullptr;   // [nz*ny][2 nx]
     float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]
+    CUtensorMap conv_map;   // tensor map of the array k_conv transforms in place (W1 in 2-D, W2 in 3-D)
     float *abl[3] = {nullptr, nullptr, nullptr};
     double *norms = nullptr, *history = nullptr;
     int hist_cap = 0;
@@ -125,7 +126,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = a.out_line_stride = mx;
         a.p2_line = (const float2 *)f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
-        if (which < 0 || which == 0) e = launch_conv(ny, a, 1, st);
+        if (which < 0 || which == 0) e = launch_conv(ny, a, &pl->conv_map, 1, st);
         return e;
     }
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
@@ -144,7 +145,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
         a.p2_line = (const float2 *)f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
-        e = launch_conv(nz, a, (int)my, st);
+        e = launch_conv(nz, a, &pl->conv_map, (int)my, st);
         if (e != cudaSuccess) return e;
     }
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
@@ -175,10 +176,10 @@ cudaError_t set_kernel_attrs(tbs_plan *pl) {
     cudaError_t e;
     if ((e = launch_row<true>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
     if ((e = launch_row<false>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
-    if (pl->ndim == 2) return launch_conv(pl->n[1], ca, 1, 0, true);
+    if (pl->ndim == 2) return launch_conv(pl->n[1], ca, nullptr, 1, 0, true);
     if ((e = launch_col<MODE_FWD>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
     if ((e = launch_col<MODE_INV>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
-    return launch_conv(pl->n[2], ca, 1, 0, true);
+    return launch_conv(pl->n[2], ca, nullptr, 1, 0, true);
 }
 
 tbs_status ensure_history(tbs_plan *pl, int max_terms) {
@@ -281,6 +282,11 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
         const long long rows = (long long)pl->n[1] * pl->n[2];
         CU(pl, dmalloc(pl, &pl->W1, (size_t)(rows * 2 * pl->n[0])));
         if (ndim == 3) CU(pl, dmalloc(pl, &pl->W2, (size_t)((long long)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0])));
+        {
+            const long long mx = 2LL * pl->n[0], my = 2LL * pl->n[1];
+            if (ndim == 2) CU(pl, make_conv_tensor_map(&pl->conv_map, pl->W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
+            else CU(pl, make_conv_tensor_map(&pl->conv_map, pl->W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
+        }
         for (int a = 0; a < ndim; ++a) {
             CU(pl, dmalloc(pl, &pl->abl[a], pl->n[a]));
             k_abl_window<<<nblk(pl->n[a], 256), 256>>>(pl->abl[a], pl->n[a], 0, 0.0);
