@@ -59,10 +59,6 @@ static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, 
     return cudaGetLastError();
 }
 
-#ifndef TBS_CONV_TMA
-#define TBS_CONV_TMA 1   // 1: input tiles through the tensor map (TMA); 0: 16-byte cp.async copies
-#endif
-
 // Tensor map of the array k_conv reads: a 2-D tensor of 8-byte elements, dim0 = all columns (x, or
 // (ky, kx) in the 3-D z pass), dim1 = the N positions along the line; box = T columns x min(N, 256) rows,
 // hardware swizzle matched to the 16-byte-chunk XOR of the staging layout.
@@ -100,7 +96,7 @@ static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int 
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = T * tpl_of(N);
     constexpr size_t smem = (size_t)conv_stage_offset(N, T) + (size_t)N * T * sizeof(float2);
-    auto kern = k_conv<N, T, ConvCfg<N>::MINB, TBS_CONV_TMA != 0>;
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
     static int cap = 0;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -382,11 +382,11 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
 }
 
 // K2 (2-D) / the z pass (3-D): for each of T adjacent lines along a strided axis: pad, FFT, .ghat,
-// IFFT, crop, in place in global memory.  Persistent; tile i+1 is fetched with
-// cp.async into a staging buffer while tile i computes; the result goes back through the work area
-// so that global reads and writes are 16 bytes per lane over adjacent lines.  Between the three
-// CTA-wide barriers of a tile the T line groups run on their own barriers.
-template <int N, int T, int MINB, bool USE_TMA>
+// IFFT, crop, in place in global memory.  Persistent.  Tiles move by TMA: tile i+1
+// is fetched through the tensor map into a staging buffer while tile i computes, and the result tile
+// is stored through the same map.  Between the four CTA-wide barriers of a tile the T line groups run
+// on their own barriers.
+template <int N, int T, int MINB>
 __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
@@ -395,14 +395,15 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     constexpr int TPL = tpl_of(N);
     constexpr int NT = T * TPL;
     constexpr int GT = TPL >= 32 ? TPL : 32;
+    constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
     using Lay = LineLay<N, conv_pad(N, T)>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
     // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
-    // 2c+1), the chunk index XOR-swizzled with the position so that the cp.async writes of a warp are
-    // contiguous and the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
+    // 2c+1), the chunk index XOR-swizzled with the position (the TMA swizzle mode of that row width)
+    // so that the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
     float4 *stg = wk + conv_stage_offset(N, T) / 16;  // 1024-byte aligned (TMA swizzle atom)
     __shared__ __align__(8) uint64_t mbar;
     if (a.ctl->done) return;
@@ -414,25 +415,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     const int total = tiles * a.n_outer;
     auto swz = [](int r) { return CPR > 1 ? (r / (CPR >= 8 ? 1 : 8 / CPR)) % CPR : 0; };
 
-    // part q of NQ of the cp.async copies of one tile (spread over the phases of the previous tile)
-    constexpr int NQ = 4;
-    static_assert((N * CPR) % (NT * NQ) == 0 || N * CPR < NT * NQ, "staging split");
-    auto stage_part = [&](int tile, int q) {
-        const float2 *src = a.in + (long long)(tile / tiles) * a.in_outer_stride + (tile % tiles) * T;
-        constexpr int PER = (N * CPR + NQ - 1) / NQ;
-#pragma unroll 2
-        for (int c = q * PER + tid; c < (q + 1) * PER && c < N * CPR; c += NT) {
-            const int r = c / CPR, cc = c % CPR;
-            cp_async16(stg + r * CPR + (cc ^ swz(r)), src + (long long)r * a.in_line_stride + 2 * cc);
-        }
-    };
-    auto stage_tile = [&](int tile) {
-#pragma unroll
-        for (int q = 0; q < NQ; ++q) stage_part(tile, q);
-        cp_async_commit();
-    };
-    // USE_TMA: the same tile arrives as N/BR boxes of BR rows x T columns through the tensor map
-    // (cp.async.bulk.tensor, hardware swizzle = the XOR above), issued by one thread, completion on mbar.
+    // A tile arrives as N/BR boxes of BR rows x T columns through the tensor map (cp.async.bulk.tensor,
+    // hardware swizzle = the XOR above), issued by one thread a tile ahead, completion on mbar; the
+    // result leaves the same way from a dense tile written over the (then dead) work area.
     constexpr int BR = N < 256 ? N : 256;
     constexpr uint32_t TILE_BYTES = (uint32_t)N * T * sizeof(float2);
     uint32_t phase = 0;
@@ -442,11 +427,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
 #pragma unroll 1
         for (int k = 0; k < N / BR; ++k) tma_load_2d(stg + k * BR * CPR, &tmap, c0, k * BR, &mbar);
     };
-    if (USE_TMA) {
-        if (tid == 0) mbar_init(&mbar, 1);
-        __syncthreads();
-        if (tid == 0 && (int)blockIdx.x < total) tma_tile(blockIdx.x);
-    } else if ((int)blockIdx.x < total) stage_tile(blockIdx.x);
+    if (tid == 0) mbar_init(&mbar, 1);
+    __syncthreads();
+    if (tid == 0 && (int)blockIdx.x < total) tma_tile(blockIdx.x);
     const float2 *stg2 = reinterpret_cast<const float2 *>(stg) + (line & 1);
 
 #pragma unroll 1
@@ -454,13 +437,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         const int inner0 = (tile % tiles) * T;
         const int outer = tile / tiles;
         const bool more = tile + (int)gridDim.x < total;
-        if (USE_TMA) {
-            mbar_wait(&mbar, phase);
-            phase ^= 1u;
-        } else {
-            cp_async_wait_all();
-        }
-        __syncthreads();  // staged tile visible; the copy-out of the previous tile has left the work area
+        mbar_wait(&mbar, phase);
+        phase ^= 1u;
+        __syncthreads();  // staged tile visible; thread 0 has seen the previous result tile leave shared memory
         // ---- forward: N inputs -> both halves ----
 #pragma unroll 1
         for (int t = lt; t < S1; t += TPL) {
@@ -473,10 +452,7 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
         }
         __syncthreads();  // staging buffer free (and the line groups are in step)
-        // the cp.async copies of the next tile are issued in four parts, one after each stage
-        if (USE_TMA) {
-            if (more && tid == 0) tma_tile(tile + gridDim.x);
-        } else if (more) stage_part(tile + gridDim.x, 0);
+        if (more && tid == 0) tma_tile(tile + gridDim.x);
         if (R2 > 0) {
             pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, line, lt);
             group_sync<GT>(g);
@@ -487,40 +463,42 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             a_line *= a.inv_e;
 #pragma unroll 1
             for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line);
-            if (!USE_TMA && more) stage_part(tile + gridDim.x, 1);
             group_sync<GT>(g);
         }
-        // ---- inverse: both halves -> N outputs, left in the first 8 bytes of their slots ----
+        // ---- inverse: both halves -> N outputs ----
         if (R2 > 0) {
             pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, line, lt);
-            if (!USE_TMA && more) stage_part(tile + gridDim.x, 2);
             group_sync<GT>(g);
-        } else if (!USE_TMA && more) {
-            stage_part(tile + gridDim.x, 2);
         }
-#pragma unroll 1
-        for (int t = lt; t < S1; t += TPL) {
-            float2 z[R1];
-            plast_inv<N, R1, Lay>(z, line, t, wk, a.lut.AB);
+        {
+            float2 z[NITEM][R1];
 #pragma unroll
-            for (int j = 0; j < R1; ++j) *reinterpret_cast<float2 *>(wk + Lay::addr(line, t + j * S1)) = z[j];
+            for (int it = 0; it < NITEM; ++it) {
+                if (it > 0) asm volatile("" ::: "memory");  // one item at a time: keeps the register peak down
+                plast_inv<N, R1, Lay>(z[it], line, lt + it * TPL, wk, a.lut.AB);
+            }
+            __syncthreads();  // every slot of the work area has been read
+            // result tile, dense [N][T] with the staging swizzle, over the start of the work area
+            float2 *o2 = reinterpret_cast<float2 *>(wk) + (line & 1);
+#pragma unroll
+            for (int it = 0; it < NITEM; ++it)
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const int r = lt + it * TPL + j * S1;
+                    o2[2 * (r * CPR + ((line >> 1) ^ swz(r)))] = z[it][j];
+                }
         }
-        if (!USE_TMA && more) {
-            stage_part(tile + gridDim.x, 3);
-            cp_async_commit();
-        }
+        fence_async_smem();
         __syncthreads();
-        float2 *dst = a.out + (long long)outer * a.out_outer_stride + inner0;
-        // lanes: 4 (or CPR) adjacent chunks x 8 positions, conflict-free with the line pitch of conv_pad
-        constexpr int CL = CPR < 4 ? CPR : 4;
-#pragma unroll 4
-        for (int c = tid; c < N * CPR; c += NT) {
-            const int r = (c / CL) % N, cc = (c / (CL * N)) * CL + c % CL;
-            const float2 v0 = *reinterpret_cast<const float2 *>(wk + Lay::addr(2 * cc, r));
-            const float2 v1 = *reinterpret_cast<const float2 *>(wk + Lay::addr(2 * cc + 1, r));
-            *reinterpret_cast<float4 *>(dst + (long long)r * a.out_line_stride + 2 * cc) = make_float4(v0.x, v0.y, v1.x, v1.y);
+        if (tid == 0) {
+            const int c0 = outer * (int)a.out_outer_stride + inner0;
+#pragma unroll 1
+            for (int k = 0; k < N / BR; ++k) tma_store_2d(&tmap, wk + k * BR * CPR, c0, k * BR);
+            bulk_commit();
+            bulk_wait_read();  // the next tile's first stage overwrites the work area
         }
     }
+    if (tid == 0) bulk_wait_all();
 }
 
 }  // namespace tbs
