@@ -95,7 +95,7 @@ template <int N>
 static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr) {
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = T * tpl_of(N);
-    constexpr size_t smem = (size_t)conv_stage_offset(N, T) + (size_t)N * T * sizeof(float2);
+    constexpr size_t smem = (size_t)conv_smem_bytes(N, T);
     auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
     static int cap = 0;
     if (set_attr) {

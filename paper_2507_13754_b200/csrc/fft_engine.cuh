@@ -148,10 +148,11 @@ struct Luts {
 };
 
 // K0 = 1 skips k = 0 (the twiddle is 1 in tables A and C).
-template <int R, int S, int K0>
+// SM = true: the table is a shared-memory copy (plain loads); false: global memory through L1.
+template <int R, int S, int K0, bool SM = false>
 __device__ __forceinline__ void load_tw(float2 (&w)[R], const float2 *__restrict__ lut, int t) {
 #pragma unroll
-    for (int k = K0; k < R; ++k) w[k] = __ldg(lut + k * S + t);
+    for (int k = K0; k < R; ++k) w[k] = SM ? lut[k * S + t] : __ldg(lut + k * S + t);
 }
 
 // d * w_32^(idx) with sign SGN; idx in [0, 16).
@@ -216,6 +217,16 @@ __host__ __device__ constexpr int conv_pad(int N, int T) {
 // Byte offset of k_conv's staging buffer behind its work area, rounded to the 1024-byte swizzle atom.
 __host__ __device__ constexpr int conv_stage_offset(int N, int T) {
     return (T * (N + N / 16 + conv_pad(N, T)) * 16 + 1023) / 1024 * 1024;
+}
+// k_conv shared memory: work area, staging, the middle-stage twiddle table C (N/R1 entries, plans with
+// three stages) and -- when that leaves the CTA under 128 KB, so that L1 keeps room for the first/last-
+// stage table (measured: at N = 2048 the copy costs more in L1 misses than it saves) -- the line-axis table.
+__host__ __device__ constexpr int conv_lutc_entries(int N) { return N >= 512 ? N / 8 : 0; }
+__host__ __device__ constexpr bool conv_p2_in_smem(int N, int T) {
+    return conv_stage_offset(N, T) + N * T * 8 + conv_lutc_entries(N) * 8 + N * 8 <= 128 * 1024;
+}
+__host__ __device__ constexpr int conv_smem_bytes(int N, int T) {
+    return conv_stage_offset(N, T) + N * T * 8 + (conv_p2_in_smem(N, T) ? conv_lutc_entries(N) * 8 + N * 8 : 0);
 }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
 template <int GT>

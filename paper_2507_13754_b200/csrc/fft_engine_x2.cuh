@@ -118,18 +118,18 @@ __device__ __forceinline__ void pstage_item_tw(float4 *sm, const float2 (&tw)[R]
         for (int i = 0; i < R; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, R) * S), v[i]);
     }
 }
-template <int N, int LB, int R, bool FWD, class Lay>
+template <int N, int LB, int R, bool FWD, class Lay, bool TSM = false>
 __device__ __forceinline__ void pstage_item(float4 *sm, const float2 *__restrict__ lut, int line, int b) {
     constexpr int S = LB / R;
     float2 tw[R];
-    if (S > 1) load_tw<R, S, 1>(tw, lut, b % S);
+    if (S > 1) load_tw<R, S, 1, TSM>(tw, lut, b % S);
     pstage_item_tw<N, LB, R, FWD, Lay>(sm, tw, line, b);
 }
-template <int N, int LB, int R, bool FWD, class Lay, int TPL>
+template <int N, int LB, int R, bool FWD, class Lay, int TPL, bool TSM = false>
 __device__ __forceinline__ void pstage_line(float4 *sm, const float2 *__restrict__ lut, int line, int lt) {
     constexpr int NBL = N / R;
 #pragma unroll 1
-    for (int b = lt; b < NBL; b += TPL) pstage_item<N, LB, R, FWD, Lay>(sm, lut, line, b);
+    for (int b = lt; b < NBL; b += TPL) pstage_item<N, LB, R, FWD, Lay, TSM>(sm, lut, line, b);
 }
 
 // Interleaved first/last-stage table: lutAB[k][t] = (A.x, B.x, A.y, B.y) with A = w_N^(k t) (even
@@ -207,17 +207,17 @@ __device__ __forceinline__ void plast_inv(float2 (&z)[R1], int line, int t, cons
 // and one MUFU.RCP per half; the constant 1/(e k0^2) rides on the normalisation applied by k_row.
 // p2x2: the line-axis table |p|^2/(e k0^2), interleaved over the halves, [j][block] float2 = (even, odd);
 // a_line: (|p|^2 of the other axes / k0^2 - 1) / e.
-template <int N, int RL>
+template <int N, int RL, bool TSM>
 __device__ __forceinline__ void load_p2x2(float2 (&pp)[RL], const float2 *__restrict__ p2x2, int b) {
 #pragma unroll
-    for (int j = 0; j < RL; ++j) pp[j] = __ldg(p2x2 + j * (N / RL) + b);
+    for (int j = 0; j < RL; ++j) pp[j] = TSM ? p2x2[j * (N / RL) + b] : __ldg(p2x2 + j * (N / RL) + b);
 }
-template <int N, int RL, class Lay>
+template <int N, int RL, class Lay, bool TSM = false>
 __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
                                                float a_line) {
     const int base = b * RL;
     float2 pp[RL];
-    load_p2x2<N, RL>(pp, p2x2, b);
+    load_p2x2<N, RL, TSM>(pp, p2x2, b);
     P2 v[RL];
 #pragma unroll
     for (int j = 0; j < RL; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j));

@@ -406,6 +406,11 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     // so that the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
     float4 *stg = wk + conv_stage_offset(N, T) / 16;  // 1024-byte aligned (TMA swizzle atom)
     __shared__ __align__(8) uint64_t mbar;
+    // Shared-memory copies of the tables every tile re-reads, for the tile shapes that leave room
+    // (fft_engine.cuh, conv_p2_in_smem): the middle-stage twiddles C and the line-axis spectrum table.
+    constexpr bool P2SM = conv_p2_in_smem(N, T);
+    float2 *lutC_s = reinterpret_cast<float2 *>(stg + N * CPR);
+    float2 *p2_s = lutC_s + (R2 > 0 ? S1 : 0);
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
@@ -428,6 +433,13 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         for (int k = 0; k < N / BR; ++k) tma_load_2d(stg + k * BR * CPR, &tmap, c0, k * BR, &mbar);
     };
     if (tid == 0) mbar_init(&mbar, 1);
+    if (P2SM) {
+        if (R2 > 0)
+            for (int i = tid; i < S1; i += NT) lutC_s[i] = __ldg(a.lut.C + i);
+        for (int i = tid; i < N; i += NT) p2_s[i] = __ldg(a.p2_line + i);
+    }
+    const float2 *p2_tab = P2SM ? p2_s : a.p2_line;
+    const float2 *lutC_tab = P2SM ? lutC_s : a.lut.C;
     __syncthreads();
     if (tid == 0 && (int)blockIdx.x < total) tma_tile(blockIdx.x);
     const float2 *stg2 = reinterpret_cast<const float2 *>(stg) + (line & 1);
@@ -454,7 +466,7 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         __syncthreads();  // staging buffer free (and the line groups are in step)
         if (more && tid == 0) tma_tile(tile + gridDim.x);
         if (R2 > 0) {
-            pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, line, lt);
+            pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             group_sync<GT>(g);
         }
         {
@@ -462,12 +474,12 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
             a_line *= a.inv_e;
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay>(wk, line, b, a.p2_line, a_line);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM>(wk, line, b, p2_tab, a_line);
             group_sync<GT>(g);
         }
         // ---- inverse: both halves -> N outputs ----
         if (R2 > 0) {
-            pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, line, lt);
+            pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             group_sync<GT>(g);
         }
         {
