@@ -15,14 +15,14 @@ template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
 
 // Row kernel k_row: GROUPS independent line groups per CTA (a group = N/16 threads on one row, or
 // one warp on 32/(N/16) rows), at least MINB CTAs per SM (register cap).  Shared memory per row =
-// (N + N/16)*16 bytes of work area + N*16 bytes of W staging.  Values measured on B200 (cfg2-cfg5).
+// N*16 bytes of work area + N*16 bytes of W staging.  Values measured on B200 (cfg2-cfg5).
 template <int N> struct RowCfg { static constexpr int GROUPS = 4, MINB = 2; };   // N <= 512
 template <> struct RowCfg<1024> { static constexpr int GROUPS = 2, MINB = 3; };
 template <> struct RowCfg<2048> { static constexpr int GROUPS = 1, MINB = 3; };
 template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 1; };
 
 // Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads, at least MINB CTAs
-// per SM.  Shared memory = T*(N + N/16 + pad)*16 bytes of work area + N*T*8 bytes of input staging.
+// per SM.  Shared memory = T*N*16 bytes of work area + N*T*8 bytes of input staging (+ tables).
 template <int N> struct ConvCfg { static constexpr int T = 16, MINB = 2; };    // N < 256
 template <> struct ConvCfg<256>  { static constexpr int T = 8, MINB = 3; };
 template <> struct ConvCfg<512>  { static constexpr int T = 8, MINB = 2; };

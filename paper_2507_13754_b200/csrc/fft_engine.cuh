@@ -209,14 +209,9 @@ struct RowLay {
 // Threads that own one line in the line-group kernels (k_row, k_conv): one radix-16 item each in
 // the widest stage.  Groups of TPL >= 32 threads synchronise on a named barrier of their own,
 // smaller groups share a warp and use __syncwarp, so no stage waits for the whole CTA.
-// Extra slots per line of the k_conv work area (16-byte slots): the cooperative copy-out reads, per
-// half-warp, 4 line pairs x 4 positions when T >= 8; a pitch of 2 modulo 8 spreads them evenly.
-__host__ __device__ constexpr int conv_pad(int N, int T) {
-    return T >= 8 ? (2 + 16 - (N + N / 16) % 8) % 8 : 0;
-}
 // Byte offset of k_conv's staging buffer behind its work area, rounded to the 1024-byte swizzle atom.
 __host__ __device__ constexpr int conv_stage_offset(int N, int T) {
-    return (T * (N + N / 16 + conv_pad(N, T)) * 16 + 1023) / 1024 * 1024;
+    return (T * N * 16 + 1023) / 1024 * 1024;
 }
 // k_conv shared memory: work area, staging, the middle-stage twiddle table C (N/R1 entries, plans with
 // three stages) and -- when that leaves the CTA under 128 KB, so that L1 keeps room for the first/last-

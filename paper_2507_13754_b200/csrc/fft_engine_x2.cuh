@@ -81,11 +81,14 @@ __device__ __forceinline__ P2 lds_p2(const float4 *p) {
 }
 __device__ __forceinline__ void sts_p2(float4 *p, P2 v) { *p = make_float4(v.re.x, v.re.y, v.im.x, v.im.y); }
 
-// Packed line layout: one float4 per position, one pad slot per 16 positions, PAD extra per line.
-template <int N, int PAD = 0>
+// Packed line layout: one float4 (16-byte slot) per position, N slots per line, no padding.  The slot
+// index is the position with bits 4-6 XORed into bits 0-2: every access pattern of the stages (threads
+// on consecutive positions; threads on consecutive blocks of 16 reading the same offset; strides of 16
+// inside a block of 256) then touches 8 different 16-byte banks per quarter-warp.
+template <int N>
 struct LineLay {
-    static constexpr int PITCH = N + N / 16 + PAD;
-    __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + pos + (pos >> 4); }
+    static constexpr int PITCH = N;
+    __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + (pos ^ ((pos >> 4) & 7)); }
 };
 
 // In-place stage (block length LB, radix R, sub-stride S = LB/R) of one item of one line.

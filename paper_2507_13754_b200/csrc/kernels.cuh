@@ -398,7 +398,7 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
-    using Lay = LineLay<N, conv_pad(N, T)>;
+    using Lay = LineLay<N>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
     // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
