@@ -382,10 +382,10 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
 }
 
 // K2 (2-D) / the z pass (3-D): for each of T adjacent lines along a strided axis: pad, FFT, .ghat,
-// IFFT, crop, in place in global memory.  Persistent.  Tiles move by TMA: tile i+1
-// is fetched through the tensor map into a staging buffer while tile i computes, and the result tile
-// is stored through the same map.  Between the four CTA-wide barriers of a tile the T line groups run
-// on their own barriers.
+// IFFT, crop, in place in global memory.  Persistent.  Tiles move by TMA through one
+// tile buffer used in place for both directions; the last inverse stage of a tile is fused with the
+// first forward stage of the next one (as in k_row), so a tile costs four stages and ONE CTA-wide
+// barrier; between them the T line groups run on their own barriers.
 template <int N, int T, int MINB>
 __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
     using P = Radix<N>;
@@ -421,8 +421,8 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     auto swz = [](int r) { return CPR > 1 ? (r / (CPR >= 8 ? 1 : 8 / CPR)) % CPR : 0; };
 
     // A tile arrives as N/BR boxes of BR rows x T columns through the tensor map (cp.async.bulk.tensor,
-    // hardware swizzle = the XOR above), issued by one thread a tile ahead, completion on mbar; the
-    // result leaves the same way from a dense tile written over the (then dead) work area.
+    // hardware swizzle = the XOR above), issued by one thread, completion on mbar; the result leaves the
+    // same way from the same buffer.
     constexpr int BR = N < 256 ? N : 256;
     constexpr uint32_t TILE_BYTES = (uint32_t)N * T * sizeof(float2);
     uint32_t phase = 0;
@@ -441,33 +441,51 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     const float2 *p2_tab = P2SM ? p2_s : a.p2_line;
     const float2 *lutC_tab = P2SM ? lutC_s : a.lut.C;
     __syncthreads();
-    if (tid == 0 && (int)blockIdx.x < total) tma_tile(blockIdx.x);
-    const float2 *stg2 = reinterpret_cast<const float2 *>(stg) + (line & 1);
+    // I/O element of this thread's line at position r of the tile buffer
+    float2 *io = reinterpret_cast<float2 *>(stg) + (line & 1);
+    auto io_at = [&](int r) -> float2 & { return io[2 * (r * CPR + ((line >> 1) ^ swz(r)))]; };
+    auto store_tile = [&](int tile) {
+        const int c0 = (tile / tiles) * (int)a.out_outer_stride + (tile % tiles) * T;
+#pragma unroll 1
+        for (int k = 0; k < N / BR; ++k) tma_store_2d(&tmap, stg + k * BR * CPR, c0, k * BR);
+        bulk_commit();
+    };
+
+    // The tile buffer serves both directions, in place: in the fused last/first stage a thread reads
+    // the next tile's input at its positions and leaves the current tile's result there.  Thread 0
+    // stores the buffer and refills it, once the store has been read out, for the tile after next:
+    // under the first middle stage of the next tile (three-stage plans), else at once.
+    int tile = blockIdx.x;
+    if (tile >= total) return;
+    if (tid == 0) tma_tile(tile);
+    // ---- prologue: first stage of the first tile ----
+    mbar_wait(&mbar, phase);
+    phase ^= 1u;
+#pragma unroll 1
+    for (int t = lt; t < S1; t += TPL) {
+        float2 x[R1];
+#pragma unroll
+        for (int j = 0; j < R1; ++j) x[j] = io_at(t + j * S1);
+        pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
+    }
+    __syncthreads();
+    int to_load = tile + 2 * (int)gridDim.x < total ? tile + 2 * (int)gridDim.x : -1;  // refill after the next store
+    if (tid == 0 && tile + (int)gridDim.x < total) tma_tile(tile + gridDim.x);
 
 #pragma unroll 1
-    for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+    for (; tile < total; tile += gridDim.x) {
         const int inner0 = (tile % tiles) * T;
         const int outer = tile / tiles;
         const bool more = tile + (int)gridDim.x < total;
-        mbar_wait(&mbar, phase);
-        phase ^= 1u;
-        __syncthreads();  // staged tile visible; thread 0 has seen the previous result tile leave shared memory
-        // ---- forward: N inputs -> both halves ----
-#pragma unroll 1
-        for (int t = lt; t < S1; t += TPL) {
-            float2 x[R1];
-#pragma unroll
-            for (int j = 0; j < R1; ++j) {
-                const int r = t + j * S1;
-                x[j] = stg2[2 * (r * CPR + ((line >> 1) ^ swz(r)))];
-            }
-            pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
-        }
-        __syncthreads();  // staging buffer free (and the line groups are in step)
-        if (more && tid == 0) tma_tile(tile + gridDim.x);
         if (R2 > 0) {
             pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             group_sync<GT>(g);
+            // by now the store of the previous tile has been read out of the buffer: refill it
+            if (tid == 0 && to_load >= 0 && tile != (int)blockIdx.x) {
+                bulk_wait_read();
+                tma_tile(to_load);
+            }
+            if (tile != (int)blockIdx.x) to_load = to_load >= 0 && to_load + (int)gridDim.x < total ? to_load + (int)gridDim.x : -1;
         }
         {
             float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
@@ -477,38 +495,39 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM>(wk, line, b, p2_tab, a_line);
             group_sync<GT>(g);
         }
-        // ---- inverse: both halves -> N outputs ----
         if (R2 > 0) {
             pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             group_sync<GT>(g);
         }
-        {
-            float2 z[NITEM][R1];
+        // ---- fused: last inverse stage of this tile, first forward stage of the next one ----
+        if (more) {
+            mbar_wait(&mbar, phase);
+            phase ^= 1u;
+        }
+#pragma unroll 1
+        for (int t = lt; t < S1; t += TPL) {
+            float2 wre[R1], wim[R1];
+            load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
+            float2 z[R1], x[R1];
+            plast_inv_tw<N, R1, Lay>(z, line, t, wk, wre, wim);
 #pragma unroll
-            for (int it = 0; it < NITEM; ++it) {
-                if (it > 0) asm volatile("" ::: "memory");  // one item at a time: keeps the register peak down
-                plast_inv<N, R1, Lay>(z[it], line, lt + it * TPL, wk, a.lut.AB);
+            for (int j = 0; j < R1; ++j) {
+                float2 &e = io_at(t + j * S1);
+                x[j] = e;
+                e = z[j];
             }
-            __syncthreads();  // every slot of the work area has been read
-            // result tile, dense [N][T] with the staging swizzle, over the start of the work area
-            float2 *o2 = reinterpret_cast<float2 *>(wk) + (line & 1);
-#pragma unroll
-            for (int it = 0; it < NITEM; ++it)
-#pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    const int r = lt + it * TPL + j * S1;
-                    o2[2 * (r * CPR + ((line >> 1) ^ swz(r)))] = z[it][j];
-                }
+            if (more) pfirst_fwd_tw<N, R1, Lay>(x, line, t, wk, wre, wim);
         }
         fence_async_smem();
-        __syncthreads();
+        __syncthreads();  // result tile complete, next input consumed, next first stage in place
         if (tid == 0) {
-            const int c0 = outer * (int)a.out_outer_stride + inner0;
-#pragma unroll 1
-            for (int k = 0; k < N / BR; ++k) tma_store_2d(&tmap, wk + k * BR * CPR, c0, k * BR);
-            bulk_commit();
-            bulk_wait_read();  // the next tile's first stage overwrites the work area
+            store_tile(tile);
+            if (R2 == 0 && to_load >= 0) {  // two-stage plans: no stage to hide the drain under
+                bulk_wait_read();
+                tma_tile(to_load);
+            }
         }
+        if (R2 == 0) to_load = to_load >= 0 && to_load + (int)gridDim.x < total ? to_load + (int)gridDim.x : -1;
     }
     if (tid == 0) bulk_wait_all();
 }
