@@ -27,6 +27,7 @@ struct Ctl {
     double tol;
     unsigned int ticket;  // CTAs of the current k_row launch that have finished
     int n_terms;     // index of the last term added
+    unsigned int next_tile;  // k_row: row tiles handed out beyond the first one of every group
 };
 
 enum { MODE_FWD = 1, MODE_INV = 2 };
@@ -215,6 +216,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     float4 *stg = wk + ROWS * Lay::PITCH;         // [ROWS][N] staged W rows
     __shared__ float red[2][32];
     __shared__ __align__(8) uint64_t mbar[GROUPS];
+    __shared__ int next_gt[GROUPS];
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
@@ -239,8 +241,10 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
         }
     }
 
+    // Every group starts on tile B*GROUPS + G; further tiles are handed out by an atomic counter (the
+    // groups of a launch do not finish their rows at the same pace; FIRST keeps the static walk).
 #pragma unroll 1
-    for (; gt < ngt; gt += gstride) {
+    while (gt < ngt) {
         const int row = gt * GR + gl / TPL;
         float wrow = a.scale;
         float2 pold[NITEM][R1], vpot[NITEM][R1];
@@ -269,10 +273,14 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 for (int i = 0; i < RL; ++i) sts_p2(wk + Lay::addr(l, b * RL + brev(i, RL)), v[i]);
             }
             group_sync<GT>(g);
-            // the group's staging rows are free: fetch the W rows of its next tile
-            if (gl == 0 && gt + gstride < ngt) {
-                mbar_expect_tx(&mbar[g], TILE_BYTES);
-                bulk_g2s(stg + g * GR * N, a.W + (long long)(gt + gstride) * GR * M, TILE_BYTES, &mbar[g]);
+            // the group's staging rows are free: take the next tile and fetch its W rows
+            if (gl == 0) {
+                const int nxt = gstride + (int)atomicAdd(&a.ctl->next_tile, 1u);
+                next_gt[g] = nxt;
+                if (nxt < ngt) {
+                    mbar_expect_tx(&mbar[g], TILE_BYTES);
+                    bulk_g2s(stg + g * GR * N, a.W + (long long)nxt * GR * M, TILE_BYTES, &mbar[g]);
+                }
             }
             if (R2 > 0) pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
             // request the running field and the potential at the thread's output points now: their
@@ -321,7 +329,11 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             pfirst_fwd_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
         }
         group_sync<GT>(g);
-        if (!FIRST && !a.do_fwd) continue;
+        const int gt_next = FIRST ? gt + gstride : next_gt[g];
+        if (!FIRST && !a.do_fwd) {
+            gt = gt_next;
+            continue;
+        }
         // ---------------- forward half: the remaining stages of FFT_x ----------------
         if (R2 > 0) {
             pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, l, lt);
@@ -341,6 +353,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 gp[brev(i, RL) * NBL] = make_float4(v[i].re.x, v[i].im.x, v[i].re.y, v[i].im.y);
         }
         if (FIRST) group_sync<GT>(g);  // the next tile's first stage writes slots other threads still read
+        gt = gt_next;
     }
 
     if (!FIRST) {
@@ -367,6 +380,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 const double r = sqrt(nu) / sqrt(np);
                 a.history[term] = (term == 0) ? 1.0 : r;
                 a.ctl->ticket = 0;
+                a.ctl->next_tile = 0;
                 a.ctl->n_terms = term;
                 a.ctl->term = term + 1;
                 if (!(r == r) || r > 1.0e300) {
