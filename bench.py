@@ -37,11 +37,11 @@ ALG_BYTES = {2: {"k_row": 56.0, "k_conv": 32.0},
 #   traffic  = dram__bytes_read.sum + dram__bytes_write.sum
 #   fp32_res = FP32 results issued (packed instructions count twice), from smsp__inst_executed x mix
 NCU = {
-    "cfg3": {"k_conv": {"traffic": 67.21e6 + 15.74e6, "fp32_res": 36.50e6 * 32 * (2 * 0.533 + 0.056)},
-             "k_row": {"traffic": 134.35e6 + 44.11e6, "fp32_res": 19.58e6 * 32 * (2 * 0.466 + 0.139)}},
-    "cfg5": {"k_conv_z": {"traffic": 536.93e6 + 482.52e6, "fp32_res": 189.25e6 * 32 * (2 * 0.593 + 0.100)},
-             "k_col_fwd_y": {"traffic": 268.47e6 + 481.02e6, "fp32_res": 80.53e6 * 32 * 0.672},
-             "k_row": {"traffic": 537.11e6 + 347.20e6, "fp32_res": 58.50e6 * 32 * (2 * 0.435 + 0.197)}},
+    "cfg3": {"k_conv": {"traffic": 67.22e6 + 17.68e6, "fp32_res": 35.74e6 * 32 * (2 * 0.545 + 0.058)},
+             "k_row": {"traffic": 134.32e6 + 47.00e6, "fp32_res": 19.34e6 * 32 * (2 * 0.471 + 0.141)}},
+    "cfg5": {"k_conv_z": {"traffic": 536.93e6 + 484.54e6, "fp32_res": 193.32e6 * 32 * (2 * 0.580 + 0.098)},
+             "k_col_fwd_y": {"traffic": 268.47e6 + 479.94e6, "fp32_res": 80.53e6 * 32 * 0.672},
+             "k_row": {"traffic": 536.96e6 + 346.34e6, "fp32_res": 62.35e6 * 32 * (2 * 0.408 + 0.185)}},
 }
 FP32_PEAK = 148 * 128 * 1.965e9   # FP32 results/s: 128 lanes/clk/SM (packed f32x2 counts as 2 results, same pipe)
 
