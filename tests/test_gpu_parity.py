@@ -64,7 +64,9 @@ def test_source_deposition_matches_oracle(nd):
 
 # ------------------------------------------------------------------ one application of G (S1-S3)
 @pytest.mark.parametrize("shape", [(32, 32), (64, 128), (128, 64), (256, 256), (512, 512), (1024, 32),
-                                   (32, 32, 32), (32, 64, 128), (128, 32, 64)])
+                                   (32, 1024), (2048, 32), (32, 2048), (4096, 32), (32, 4096),
+                                   (32, 32, 32), (32, 64, 128), (128, 32, 64), (512, 32, 32), (32, 512, 32),
+                                   (256, 32, 64), (64, 256, 32)])
 def test_apply_green_matches_oracle(shape):
     rng = np.random.default_rng(sum(shape))
     x = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
