@@ -200,3 +200,40 @@ def harmonic_source(h: int, fields, beta: float, rho0: float, c0: float, f1_hz: 
     rc = lib().tbs_ref_harmonic_source(fs[0].size, int(h), ptrs, beta, rho0, c0, f1_hz, _dp(S))
     assert rc == OK, rc
     return S
+
+
+def solve_cbs(V, S, ghat, eps_nd: float, max_terms: int, tol: float, pad: int = 2, windows=None) -> RefResult:
+    """Convergent Born series (PAPER.md:25, 445, 475 name it, its ref. [16] defines it):
+    preconditioner gamma = i V / eps, psi <- psi + gamma (G(V psi + S) - psi).  In term form, with
+    M = gamma G V + 1 - gamma:   u_0 = gamma A G S,   u_{n+1} = (1 - gamma) u_n + gamma A G(V u_n),   p = sum u_n.
+    V and eps_nd in the same units (both divided by k0^2, or both not).  Plain numpy on top of apply_G;
+    stopping rule and history as in solve().  For V = -i eps (homogeneous, lossless) gamma = 1 and the
+    iterates are those of the traditional series."""
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    S = np.ascontiguousarray(S, dtype=np.complex128)
+    A = np.ones(V.shape)
+    if windows is not None:
+        nd = V.ndim
+        for a in range(nd):
+            shp = [1] * nd
+            shp[nd - 1 - a] = -1
+            A = A * np.asarray(windows[a], dtype=np.float64).reshape(shp)
+    gamma = 1j * V / eps_nd
+    u = gamma * (A * apply_G(S, ghat, pad))
+    p = u.copy()
+    hist = [1.0]
+    status, k = NOT_CONVERGED, 0
+    if max_terms == 0:
+        return RefResult(status, p, np.array(hist), 0, u)
+    for k in range(1, max_terms + 1):
+        u = (1.0 - gamma) * u + gamma * (A * apply_G(V * u, ghat, pad))
+        p += u
+        r = math.sqrt(float(np.vdot(u, u).real)) / math.sqrt(float(np.vdot(p, p).real))
+        hist.append(r)
+        if not math.isfinite(r):
+            status = ERR_DIVERGED
+            break
+        if r < tol:
+            status = OK
+            break
+    return RefResult(status, p, np.array(hist), k, u)

@@ -1,0 +1,75 @@
+"""Pins of the oracle's convergent Born series.  The paper names the scheme and its
+convergence condition and leaves the formula to its ref. [16]; what pins the oracle
+here is mathematics, not that reference: the fixed point is the solution of the same linear system as the
+traditional series (dense direct solve), the iteration matrix is M = gamma G V + 1 - gamma, and for a
+homogeneous lossless medium gamma = 1 makes the two schemes identical.  CPU only."""
+import numpy as np
+
+import oracle.tbs_ref as R
+from test_oracle_pins_c import _dense_G
+
+
+def _strong_problem(N, ratio):
+    """Large slow disc: k^2/k0^2 - 1 = ratio^2 - 1 inside (below the damping 0.8 for ratio < 1.34)."""
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / 6.0
+    ax = np.arange(N) - (N - 1) / 2
+    yy, xx = np.meshgrid(ax, ax, indexing="ij")
+    c = np.full((N, N), c0)
+    c[np.hypot(xx, yy) < N / 3] = c0 / ratio
+    V = R.potential(c, 0.0, 1.5, f, c0, 0.8)
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    g = R.green_spectrum((2 * N, 2 * N), dx, k0, eps)
+    S = np.zeros((N, N), complex)
+    S[1, 1] = 1.0
+    S[2, N // 2] = 0.5j
+    return V, S, g, eps
+
+
+def test_cbs_equals_tbs_for_homogeneous_lossless_medium():
+    """V = -i eps  =>  gamma = i V / eps = 1  =>  M = G V: same terms, same history."""
+    N = 24
+    V, S, g, eps = _strong_problem(N, 1.0)
+    assert np.allclose(V, -1j * eps)
+    a = R.solve(V, S, g, 60, 0.0)
+    b = R.solve_cbs(V, S, g, eps, 60, 0.0)
+    assert np.abs(a.p - b.p).max() < 1e-12 * np.abs(a.p).max()
+    assert np.allclose(a.history, b.history, rtol=1e-10)
+
+
+def test_cbs_converges_to_the_dense_solution_where_the_traditional_series_diverges():
+    """eps >= max |k^2 - k0^2| is enough for CBS; the same medium has rho(G V) > 1."""
+    N = 16
+    V, S, g, eps = _strong_problem(N, 1.3)
+    assert np.abs(V + 1j * eps).max() <= eps          # |k^2 - k0^2| <= eps
+    n = N * N
+    G = _dense_G(g, (N, N))
+    GV = G * V.reshape(1, n)
+    assert np.abs(np.linalg.eigvals(GV)).max() > 1.0  # the traditional series diverges
+    tbs = R.solve(V, S, g, 400, 1e-12)
+    assert tbs.status != R.OK
+    p_dense = np.linalg.solve(np.eye(n) - GV, G @ S.reshape(n)).reshape(N, N)
+    res = R.solve_cbs(V, S, g, eps, 20000, 1e-13)
+    assert res.status == R.OK
+    assert np.linalg.norm(res.p - p_dense) < 1e-9 * np.linalg.norm(p_dense)
+    # iteration matrix M = gamma G V + 1 - gamma: contraction, and its spectral radius is the tail ratio
+    gam = (1j * V / eps).reshape(n)
+    M = gam[:, None] * GV + np.diag(1.0 - gam)
+    rho = np.abs(np.linalg.eigvals(M)).max()
+    assert rho < 1.0
+    h, k = res.history, res.n_terms
+    assert abs(h[k] / h[k - 1] - rho) < 2e-2
+
+
+def test_cbs_first_terms_follow_the_definition():
+    """u_0 = gamma G S, u_1 = (1 - gamma) u_0 + gamma G(V u_0), written out with the dense matrix."""
+    N = 12
+    V, S, g, eps = _strong_problem(N, 1.2)
+    n = N * N
+    G = _dense_G(g, (N, N))
+    gam = (1j * V / eps).reshape(n)
+    u0 = gam * (G @ S.reshape(n))
+    u1 = (1 - gam) * u0 + gam * (G @ (V.reshape(n) * u0))
+    res = R.solve_cbs(V, S, g, eps, 1, 0.0)
+    assert np.abs(res.p.reshape(n) - (u0 + u1)).max() < 1e-12 * np.abs(u0).max()
+    assert abs(res.history[1] - np.linalg.norm(u1) / np.linalg.norm(u0 + u1)) < 1e-12
