@@ -63,6 +63,15 @@ size_t tbs_plan_workspace_bytes(const tbs_plan *plan);
 /* Text of the last error on this plan (plan-owned storage, valid until the next call). */
 const char *tbs_last_error(const tbs_plan *plan);
 
+/* Iteration scheme of tbs_solve* (default TBS_SCHEME_BORN, the paper's traditional Born series,
+ * PAPER.md:156-160 Eqs. 18-19).  TBS_SCHEME_CBS is the convergent Born series the paper names as the way
+ * past strong / extended scatterers (formula from its ref. [16]): with the
+ * preconditioner gamma = i V / eps,  psi <- psi + gamma (G(V psi + S) - psi);  in term form
+ * u_0 = gamma A G S, u_{n+1} = u_n + gamma (A G(V u_n) - u_n), p = sum u_n.  Same kernels, same stopping
+ * rule; one more field of n complex64 per frequency.  Converges when eps >= max |k^2 - k0^2|. */
+enum { TBS_SCHEME_BORN = 0, TBS_SCHEME_CBS = 1 };
+tbs_status tbs_set_scheme(tbs_plan *plan, int scheme);
+
 /* Absorbing layer of Eq. 29 on all faces, `cells` wide, window
  * 1/(1+exp(-zeta (x - mu/2))) with zeta*mu/2 = zeta_half_mu (paper: 9.666).  cells = 0 (default)
  * is the pure zero-pad/crop boundary.  Folded into the crop kernel as per-axis factors. */

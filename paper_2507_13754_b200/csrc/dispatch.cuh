@@ -146,8 +146,8 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
     return cudaErrorInvalidValue;
 }
 
-template <int N, bool FIRST>
-static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr) {
+template <int N, bool FIRST, bool CBS>
+static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
     constexpr int TPL = tpl_of(N);
     constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;
@@ -155,7 +155,7 @@ static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr
     constexpr int ROWS = C::GROUPS * GR;
     constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
                             (FIRST ? 0 : (size_t)ROWS * N * sizeof(float4));
-    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST>;
+    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, CBS>;
     static int cap = 0;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -165,6 +165,16 @@ static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr
     const int tiles = (a.rows / GR + C::GROUPS - 1) / C::GROUPS;
     kern<<<(unsigned)(tiles < cap ? tiles : cap), NT, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+template <int N, bool FIRST>
+static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr) {
+    if (FIRST) return launch_row_tt<N, true, false>(a, st, set_attr);
+    if (set_attr) {
+        cudaError_t e = launch_row_tt<N, false, false>(a, st, true);
+        return e != cudaSuccess ? e : launch_row_tt<N, false, true>(a, st, true);
+    }
+    return a.ucbs ? launch_row_tt<N, false, true>(a, st, false) : launch_row_tt<N, false, false>(a, st, false);
 }
 
 template <bool FIRST>

@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     constexpr int TSTEP = NT / T;
     constexpr int HALF = N * T;
     using Lay = ColLay<N, T, RL>;
-    extern __shared__ __align__(128) float2 sm[];
+    extern __shared__ __align__(1024) float2 sm[];
     float2 *stg = sm + 2 * HALF;  // [N][T] staged input tile (CONV, FWD)
     if (a.ctl->done) return;
 
@@ -170,6 +170,8 @@ struct RowArgs {
     int rows;
     float src_scale;      // FIRST: 1/k0^2
     float scale;          // k0^2/(eps prod(2 n)): inverse-transform normalisation and the 1/e of ghat (k_conv)
+    float2 *ucbs;         // CBS scheme: [rows][N] current term u_n (read and replaced); nullptr for TBS
+    float inv_e;          // CBS: k0^2/eps
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
@@ -192,10 +194,11 @@ struct RowArgs {
 //
 // FIRST = true : forward half only, w = src * src_scale (term 0: u_0 = G S, Eq. 20)
 // FIRST = false: inverse half (K3) + forward half (K1) of the next term
+// CBS   = true : the term update of the convergent Born series instead of u = A G(V u)
 // Persistent and group-independent: group G of CTA B walks row tiles (B*GROUPS + G) + i*gridDim.x*
 // GROUPS; the W rows of its next tile arrive by one bulk copy (completion on the group's mbarrier)
 // in a staging buffer while the current tile computes.
-template <int N, int GROUPS, int MINB, bool FIRST>
+template <int N, int GROUPS, int MINB, bool FIRST, bool CBS>
 __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
@@ -211,7 +214,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(S1 % TPL == 0, "items per thread");
     using Lay = LineLay<N>;
-    extern __shared__ __align__(128) float2 sm[];
+    extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [ROWS][PITCH] work area, both halves per slot
     float4 *stg = wk + ROWS * Lay::PITCH;         // [ROWS][N] staged W rows
     __shared__ float red[2][32];
@@ -254,6 +257,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             for (int i = gl; i < GR * N / 16; i += GT) {
                 prefetch_l2(a.p + (long long)gt * GR * N + i * 16);
                 prefetch_l2(a.V + (long long)gt * GR * N + i * 16);
+                if (CBS) prefetch_l2(a.ucbs + (long long)gt * GR * N + i * 16);
             }
             wrow *= __ldg(&a.ay[row % a.ny]);
             if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
@@ -311,7 +315,14 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     const int pos = t + j * S1;
                     const long long gi = (long long)row * N + pos;
                     const float wgt = wrow * __ldg(&a.ax[pos]);
-                    const float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
+                    float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
+                    if (CBS) {
+                        // convergent Born series: u_{n+1} = u_n + gamma (A G(V u_n) - u_n), gamma = i V / eps
+                        const float2 gam = make_float2(-vpot[it][j].y * a.inv_e, vpot[it][j].x * a.inv_e);
+                        const float2 uo = term > 0 ? a.ucbs[gi] : make_float2(0.f, 0.f);
+                        u = cadd(uo, cmul(gam, csub(u, uo)));
+                        a.ucbs[gi] = u;
+                    }
                     const float2 pv = cadd(pold[it][j], u);
                     a.p[gi] = pv;
                     uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
@@ -409,7 +420,6 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     constexpr int TPL = tpl_of(N);
     constexpr int NT = T * TPL;
     constexpr int GT = TPL >= 32 ? TPL : 32;
-    constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
     using Lay = LineLay<N>;

@@ -145,6 +145,7 @@ tbs_status tbs_apply_green(tbs_plan *pl, int ifreq, const float *x, float *out, 
     CU(pl, launch_row<true>(pl->n[0], r, st));
     CU(pl, launch_mid_passes(pl, f, st));
     fill_row_args(pl, f, r, nullptr, 0.f, 0);
+    r.ucbs = nullptr;  // one plain application of G, whatever the plan's scheme
     r.p = (float2 *)out;
     r.V = f.V;  // only multiplies a value that is dropped when do_fwd = 0
     CU(pl, launch_row<false>(pl->n[0], r, st));

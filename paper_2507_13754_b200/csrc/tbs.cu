@@ -23,6 +23,7 @@ struct Freq {
     float2 *V = nullptr;      // [n] V/k0^2
     float2 *S = nullptr;      // [n] source density
     float2 *p = nullptr;      // [n] running field
+    float2 *ucbs = nullptr;   // [n] current term of the convergent Born series (allocated by tbs_set_scheme)
     float *p2[3] = {nullptr, nullptr, nullptr};  // per-axis |p|^2/k0^2, position order, [2 n[a]]
     Ctl *ctl = nullptr;
     cudaGraphExec_t graph = nullptr;
@@ -55,6 +56,7 @@ struct tbs_plan {
     cudaEvent_t ev[2] = {nullptr, nullptr}, ev_t0 = nullptr, ev_t1 = nullptr;
     size_t dev_bytes = 0;
     int graph_batch = 16;
+    int scheme = TBS_SCHEME_BORN;
     long long launches = 0;
     double loop_ms = 0;
     std::string err;
@@ -103,6 +105,8 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.ny = pl->n[1];
     a.rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
     a.src_scale = src_scale;
+    a.ucbs = pl->scheme == TBS_SCHEME_CBS ? f.ucbs : nullptr;
+    a.inv_e = (float)(1.0 / pl->damping);
     a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
     a.do_fwd = do_fwd;
     a.norms = pl->norms;
@@ -226,7 +230,7 @@ void tbs_plan_destroy(tbs_plan *pl) {
     if (!pl) return;
     destroy_graphs(pl);
     for (auto &f : pl->fr) {
-        cudaFree(f.V); cudaFree(f.S); cudaFree(f.p); cudaFree(f.ctl);
+        cudaFree(f.V); cudaFree(f.S); cudaFree(f.p); cudaFree(f.ctl); cudaFree(f.ucbs);
         for (int a = 0; a < 3; ++a) cudaFree(f.p2[a]);
     }
     for (int a = 0; a < 3; ++a) { cudaFree(pl->lutA[a]); cudaFree(pl->lutB[a]); cudaFree(pl->lutC[a]); cudaFree(pl->lutAB[a]); }
@@ -324,6 +328,16 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
         return st;
     }
     *out = pl;
+    return TBS_OK;
+}
+
+tbs_status tbs_set_scheme(tbs_plan *pl, int scheme) {
+    if (!pl || (scheme != TBS_SCHEME_BORN && scheme != TBS_SCHEME_CBS)) return TBS_ERR_INVALID_ARG;
+    if (scheme == TBS_SCHEME_CBS)
+        for (auto &f : pl->fr)
+            if (!f.ucbs) CU(pl, dmalloc(pl, &f.ucbs, (size_t)pl->npts));
+    if (scheme != pl->scheme) destroy_graphs(pl);  // the captured launches carry the scheme
+    pl->scheme = scheme;
     return TBS_OK;
 }
 

@@ -100,6 +100,11 @@ class Plan:
     def workspace_bytes(self):
         return int(self._L.tbs_plan_workspace_bytes(self._h))
 
+    def set_scheme(self, scheme):
+        """tbs_set_scheme: "born" (traditional series, default) or "cbs" (convergent Born series)."""
+        code = {"born": 0, "tbs": 0, "cbs": 1}[scheme] if isinstance(scheme, str) else int(scheme)
+        self._check(self._L.tbs_set_scheme(self._h, code))
+
     def set_abl(self, cells, zeta_half_mu=9.666):
         self._check(self._L.tbs_set_abl(self._h, int(cells), float(zeta_half_mu)))
 
