@@ -63,6 +63,21 @@ size_t tbs_plan_workspace_bytes(const tbs_plan *plan);
 /* Text of the last error on this plan (plan-owned storage, valid until the next call). */
 const char *tbs_last_error(const tbs_plan *plan);
 
+/* Boundary treatment (default TBS_BOUNDARY_PAD: zero-pad to 2N per axis, linear convolution, crop --
+ * BASELINE north_star).  TBS_BOUNDARY_PERIODIC is the paper's own: the FFTs act on the N-grid itself
+ * (Eq. 19, Alg. 1 l.36-38) and wrap-around is left to the absorbing layer of tbs_set_abl
+ * (PAPER.md:251-256).  It runs through the same kernels: only the even padded frequencies, which are the
+ * frequencies of the N-grid, keep a non-zero Green's spectrum.  Rebuilds the axis tables. */
+enum { TBS_BOUNDARY_PAD = 0, TBS_BOUNDARY_PERIODIC = 1 };
+tbs_status tbs_set_boundary(tbs_plan *plan, int boundary);
+
+/* Convergence measure r_n (history[n], compared with tol).  TBS_CRIT_L2_GRID (default, reading A8):
+ * ||u_n||_2 / ||p_n||_2 over the whole grid.  TBS_CRIT_L1_ROW: the paper's Eq. 30,
+ * sum_m |psi_{l+1}(row, m) - psi_l(row, m)| / sum_m |psi_l(row, m)| = sum |u_n| / sum |p_{n-1}| on grid row
+ * `row` (index y in 2-D, z*ny + y in 3-D); history[0] = 1. */
+enum { TBS_CRIT_L2_GRID = 0, TBS_CRIT_L1_ROW = 1 };
+tbs_status tbs_set_criterion(tbs_plan *plan, int criterion, int row);
+
 /* Iteration scheme of tbs_solve* (default TBS_SCHEME_BORN, the paper's traditional Born series,
  * PAPER.md:156-160 Eqs. 18-19).  TBS_SCHEME_CBS is the convergent Born series the paper names as the way
  * past strong / extended scatterers (formula from its ref. [16]): with the

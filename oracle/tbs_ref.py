@@ -237,3 +237,38 @@ def solve_cbs(V, S, ghat, eps_nd: float, max_terms: int, tol: float, pad: int = 
             status = OK
             break
     return RefResult(status, p, np.array(hist), k, u)
+
+
+def solve_paper_mode(V, S, ghat_periodic, max_iter: int, tol: float, row: int, windows=None) -> RefResult:
+    """Algorithm 1 l.36-47 as printed, in the paper's own Picard form on the periodic
+    N-grid (pad factor 1):  psi_in = A G S;  psi_fn = A G(V psi_in + S);  error = sum_m |psi_fn(row, m) -
+    psi_in(row, m)| / sum_m |psi_in(row, m)| (Eq. 30);  stop at the first error < tol.
+    Reading A4: the window multiplies the initial field too.  history[l] = error of iteration l, n_terms =
+    iterations done.  Rows are indexed as the flattened slow axes (y in 2-D, z*ny + y in 3-D)."""
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    S = np.ascontiguousarray(S, dtype=np.complex128)
+    A = np.ones(V.shape)
+    if windows is not None:
+        nd = V.ndim
+        for a in range(nd):
+            shp = [1] * nd
+            shp[nd - 1 - a] = -1
+            A = A * np.asarray(windows[a], dtype=np.float64).reshape(shp)
+    nx = V.shape[-1]
+    psi = A * apply_G(S, ghat_periodic, 1)
+    hist = [1.0]
+    status, l = NOT_CONVERGED, 0
+    for l in range(1, max_iter + 1):
+        new = A * apply_G(V * psi + S, ghat_periodic, 1)
+        err = float(np.abs(new.reshape(-1, nx)[row] - psi.reshape(-1, nx)[row]).sum()
+                    / np.abs(psi.reshape(-1, nx)[row]).sum())
+        u = new - psi
+        psi = new
+        hist.append(err)
+        if not math.isfinite(err):
+            status = ERR_DIVERGED
+            break
+        if err < tol:
+            status = OK
+            break
+    return RefResult(status, psi, np.array(hist), l, u if max_iter > 0 else psi)

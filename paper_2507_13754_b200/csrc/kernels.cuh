@@ -170,6 +170,8 @@ struct RowArgs {
     int rows;
     float src_scale;      // FIRST: 1/k0^2
     float scale;          // k0^2/(eps prod(2 n)): inverse-transform normalisation and the 1/e of ghat (k_conv)
+    int crit_row;         // >= 0: convergence measure of PAPER.md:258-260 Eq. 30 on this row (L1, previous field);
+                          // < 0: full-grid L2, ||u_n|| / ||p_n|| (reading A8)
     float2 *ucbs;         // CBS scheme: [rows][N] current term u_n (read and replaced); nullptr for TBS
     float inv_e;          // CBS: k0^2/eps
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
@@ -325,8 +327,13 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     }
                     const float2 pv = cadd(pold[it][j], u);
                     a.p[gi] = pv;
-                    uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
-                    pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
+                    if (a.crit_row < 0) {
+                        uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
+                        pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
+                    } else if (row == a.crit_row) {  // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row
+                        uu += sqrtf(fmaf(u.x, u.x, u.y * u.y));
+                        pp += sqrtf(fmaf(pold[it][j].x, pold[it][j].x, pold[it][j].y * pold[it][j].y));
+                    }
                     x[j] = cmul(vpot[it][j], u);
                 }
                 if (!a.do_fwd) continue;
@@ -388,7 +395,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 __threadfence();
                 const double nu = *((volatile double *)&a.norms[2 * term]);
                 const double np = *((volatile double *)&a.norms[2 * term + 1]);
-                const double r = sqrt(nu) / sqrt(np);
+                const double r = a.crit_row < 0 ? sqrt(nu) / sqrt(np) : (term == 0 ? 1.0 : nu / np);
                 a.history[term] = (term == 0) ? 1.0 : r;
                 a.ctl->ticket = 0;
                 a.ctl->next_tile = 0;

@@ -50,11 +50,13 @@ __host__ __device__ inline int freq_of_pos(int pos, int N, int r1, int r2, int r
 // Green's-spectrum axis table (Alg. 1 l.9-10, in FFT order rather than centred +
 // fftShift): p2[P] = (2 pi F~/(M dx))^2 / k0^2 for the padded-grid frequency F held at
 // index P of a transformed line, F~ = F for F < M/2, F - M otherwise.
+//   periodic = 1: see the last statement.
 //   mult = 1, or k0^2/eps for the line-axis table of k_conv (fft_engine_x2.cuh, pmid_conv_item_pp).
 //   xorder = 0 (k_col lines): P = s*N + pos, F = 2 freqN(pos) + s.
 //   xorder = 1 (W rows of k_row; line-axis table of k_conv's fused middle stage):
 //                P = 2 q + s, q = k*(N/rl) + b, pos = b*rl + k.
-__global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0, int xorder, double mult) {
+__global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx, double k0, int xorder, double mult,
+                             int periodic) {
     const int P = blockIdx.x * blockDim.x + threadIdx.x;
     const int M = 2 * N;
     if (P >= M) return;
@@ -70,7 +72,9 @@ __global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx
     const int F = 2 * freq_of_pos(pos, N, r1, r2, rl) + s;
     const double Ft = (F < M / 2) ? (double)F : (double)(F - M);
     const double p = 2.0 * 3.14159265358979323846 * Ft / ((double)M * dx);
-    p2[P] = (float)((p * p) / (k0 * k0) * mult);
+    // periodic boundary: only the even padded frequencies F = 2k exist (they are the frequencies of the
+    // unpadded N-grid); an entry of 1e18 makes ghat vanish (to 1e-18) at the odd ones in every kernel
+    p2[P] = (periodic && s == 1) ? 1.0e18f : (float)((p * p) / (k0 * k0) * mult);
 }
 
 // Full Green's spectrum in natural FFT order, ghat = ((p2-k0^2) + i eps)/((p2-k0^2)^2 + eps^2)

@@ -57,6 +57,8 @@ struct tbs_plan {
     size_t dev_bytes = 0;
     int graph_batch = 16;
     int scheme = TBS_SCHEME_BORN;
+    int boundary = TBS_BOUNDARY_PAD;
+    int crit_row = -1;
     long long launches = 0;
     double loop_ms = 0;
     std::string err;
@@ -106,8 +108,10 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
     a.src_scale = src_scale;
     a.ucbs = pl->scheme == TBS_SCHEME_CBS ? f.ucbs : nullptr;
+    a.crit_row = pl->crit_row;
     a.inv_e = (float)(1.0 / pl->damping);
     a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
+    if (pl->boundary == TBS_BOUNDARY_PERIODIC) a.scale *= (float)(1 << pl->ndim);  // the odd half carries nothing
     a.do_fwd = do_fwd;
     a.norms = pl->norms;
     a.history = pl->history;
@@ -172,6 +176,18 @@ cudaError_t launch_term(tbs_plan *pl, Freq &f, cudaStream_t st, int do_fwd = 1) 
     RowArgs r;
     fill_row_args(pl, f, r, nullptr, 0.f, do_fwd);
     return launch_row<false>(pl->n[0], r, st);
+}
+
+// Green's-spectrum axis tables of one frequency, in the order each kernel reads them (setup_kernels.cuh).
+void fill_axis_tables(tbs_plan *pl, Freq &f) {
+    for (int a = 0; a < pl->ndim; ++a) {
+        int r1, r2, rl;
+        radices_of(pl->n[a], r1, r2, rl);
+        k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, pl->dx, f.k0,
+                                                        a == 0 || a == pl->ndim - 1,
+                                                        a == pl->ndim - 1 ? 1.0 / pl->damping : 1.0,
+                                                        pl->boundary == TBS_BOUNDARY_PERIODIC);
+    }
 }
 
 cudaError_t set_kernel_attrs(tbs_plan *pl) {
@@ -309,13 +325,8 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
             CU(pl, dmalloc(pl, &f.S, (size_t)pl->npts));
             CU(pl, dmalloc(pl, &f.p, (size_t)pl->npts));
             CU(pl, dmalloc(pl, &f.ctl, 1));
-            for (int a = 0; a < ndim; ++a) {
-                int r1, r2, rl;
-                radices_of(pl->n[a], r1, r2, rl);
-                CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
-                k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, dx_m, f.k0,
-                                                                 a == 0 || a == ndim - 1, a == ndim - 1 ? 1.0 / damping : 1.0);
-            }
+            for (int a = 0; a < ndim; ++a) CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
+            fill_axis_tables(pl, f);
         }
         CU(pl, cudaDeviceSynchronize());
         return TBS_OK;
@@ -328,6 +339,24 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
         return st;
     }
     *out = pl;
+    return TBS_OK;
+}
+
+tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
+    if (!pl || (boundary != TBS_BOUNDARY_PAD && boundary != TBS_BOUNDARY_PERIODIC)) return TBS_ERR_INVALID_ARG;
+    pl->boundary = boundary;
+    for (auto &f : pl->fr) fill_axis_tables(pl, f);
+    destroy_graphs(pl);  // the captured launches carry the normalisation
+    CU(pl, cudaDeviceSynchronize());
+    return TBS_OK;
+}
+
+tbs_status tbs_set_criterion(tbs_plan *pl, int criterion, int row) {
+    if (!pl || (criterion != TBS_CRIT_L2_GRID && criterion != TBS_CRIT_L1_ROW)) return TBS_ERR_INVALID_ARG;
+    const int rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
+    if (criterion == TBS_CRIT_L1_ROW && (row < 0 || row >= rows)) return fail(pl, TBS_ERR_INVALID_ARG, "row outside the grid");
+    pl->crit_row = criterion == TBS_CRIT_L1_ROW ? row : -1;
+    destroy_graphs(pl);
     return TBS_OK;
 }
 

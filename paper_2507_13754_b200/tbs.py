@@ -105,6 +105,16 @@ class Plan:
         code = {"born": 0, "tbs": 0, "cbs": 1}[scheme] if isinstance(scheme, str) else int(scheme)
         self._check(self._L.tbs_set_scheme(self._h, code))
 
+    def set_boundary(self, boundary):
+        """tbs_set_boundary: "pad" (zero-pad/crop, default) or "periodic" (the paper's N-grid FFTs)."""
+        code = {"pad": 0, "periodic": 1}[boundary] if isinstance(boundary, str) else int(boundary)
+        self._check(self._L.tbs_set_boundary(self._h, code))
+
+    def set_criterion(self, criterion, row=0):
+        """tbs_set_criterion: "l2_grid" (default) or "l1_row" (Eq. 30 of the paper on grid row `row`)."""
+        code = {"l2_grid": 0, "l1_row": 1}[criterion] if isinstance(criterion, str) else int(criterion)
+        self._check(self._L.tbs_set_criterion(self._h, code, int(row)))
+
     def set_abl(self, cells, zeta_half_mu=9.666):
         self._check(self._L.tbs_set_abl(self._h, int(cells), float(zeta_half_mu)))
 
@@ -238,3 +248,9 @@ def solve_harmonics(plans, max_terms, tol, ref_row, surface_pressure_pa):
     res = [SolveResult(st, outs[i], hists[i], nt[i:i + 1].copy(), plans[i].last_loop_ms(), plans[i].last_launch_count())
            for i in range(nh)]
     return st, res
+
+
+def grid_harmonic_frequency(m, c0, n, dx):
+    """The m-th multiple of the fundamental frequency a periodic n-point grid supports, c0/(n dx)
+    (f = 55 v_f/(4096 dx) = 1 007 080 Hz)."""
+    return m * c0 / (n * dx)

@@ -1,0 +1,103 @@
+"""GPU parity of the paper-faithful options: periodic N-grid FFTs, the absorbing layer
+on the whole field, the centre-row L1 criterion of Eq. 30; and the paper's homogeneous case itself."""
+import numpy as np
+import pytest
+import torch
+
+import oracle.tbs_ref as R
+from parity_util import compare_fields, compare_history
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(N, abl):
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / 6.0
+    rng = np.random.default_rng(N)
+    c = (c0 * (1 + 0.01 * rng.standard_normal((N, N)))).astype(np.float32)
+    yy, xx = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    c[(xx - 0.6 * N) ** 2 + (yy - 0.5 * N) ** 2 < (N / 10) ** 2] = 1580.0
+    rows = np.arange(N // 2 - N // 8, N // 2 + N // 8 + 1)
+    pos = np.stack([np.full(rows.size, (abl + 6) * dx), rows * dx], 1)
+    amp = np.full((1, rows.size), -1.0e6j, dtype=np.complex64)
+    return f, c0, dx, c, pos, amp
+
+
+def _plan(N, abl, f, c0, dx, c, pos, amp):
+    from paper_2507_13754_b200.tbs import Plan
+    plan = Plan((N, N), dx, [f], c0, 0.8)
+    plan.set_boundary("periodic")
+    plan.set_abl(abl, 9.666)
+    plan.set_medium(torch.from_numpy(c).cuda(), alpha0_db=0.5, y=1.1)
+    plan.set_source(pos, amp)
+    return plan
+
+
+def _oracle_inputs(N, abl, f, c0, dx, c, pos, amp):
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    V = R.potential(c.astype(np.float64), 0.5, 1.1, f, c0, 0.8)
+    S = R.deposit((N, N), dx, pos, amp[0])
+    g = R.green_spectrum((N, N), dx, k0, eps)          # the N-grid itself: pad factor 1
+    win = tuple(R.abl_window(N, abl) for _ in range(2))
+    return V, S, g, win
+
+
+def test_periodic_boundary_matches_oracle_pad_factor_one():
+    N, abl = 128, 16
+    case = _case(N, abl)
+    V, S, g, win = _oracle_inputs(N, abl, *case)
+    ref = R.solve(V, S, g, 3000, 1e-6, pad=1, windows=win)
+    res = _plan(N, abl, *case).solve(3000, 1e-6)
+    assert res.status == 0 and ref.status == R.OK
+    assert abs(int(res.n_terms[0]) - ref.n_terms) <= 1
+    compare_fields(res.p[0].cpu().numpy(), ref.p, "periodic 128^2")
+
+
+def test_paper_mode_matches_oracle_algorithm_1():
+    N, abl = 256, 32
+    case = _case(N, abl)
+    V, S, g, win = _oracle_inputs(N, abl, *case)
+    ref = R.solve_paper_mode(V, S, g, 2000, 1e-5, N // 2, windows=win)
+    plan = _plan(N, abl, *case)
+    plan.set_criterion("l1_row", N // 2)
+    res = plan.solve(2000, 1e-5)
+    assert res.status == 0 and ref.status == R.OK
+    assert abs(int(res.n_terms[0]) - ref.n_terms) <= 1
+    compare_fields(res.p[0].cpu().numpy(), ref.p, "paper mode 256^2")
+    compare_history(res.history[0], ref.history, min(int(res.n_terms[0]), ref.n_terms))
+
+
+def test_paper_homogeneous_case_reproduces_table_3_iteration_count(golden):
+    """The paper's own first experiment: 4096^2 periodic grid, dx = 0.02 mm, f = the 55th
+    grid harmonic, eps = 0.8 k^2, 501-pixel line source of strength -i 10^6 at column 675 centred on row 2049,
+    450-cell sigmoid layer, Eq. 30 on row 2049 below 10^-5.  Table 3 prints 135 iterations for
+    the authors' CUDA code and 133 for their CPU code; this path must land within 10 % of them (the two
+    printed counts differ by 2; layer geometry and the window on the initial field are readings, DESIGN A4)."""
+    from paper_2507_13754_b200.tbs import Plan, grid_harmonic_frequency
+    N, dx, c0 = int(golden["n_grid"]), golden["dx_m"], golden["v_f"]
+    f = grid_harmonic_frequency(int(golden["f_multiple"]), c0, N, dx)
+    assert abs(f - golden["f_hz"]) < 0.5
+    plan = Plan((N, N), dx, [f], c0, golden["eps_over_k2"])
+    plan.set_boundary("periodic")
+    zeta_half_mu = golden["zeta_np_per_cm"] * (golden["abl_cells"] * dx * 100.0) / 2.0
+    plan.set_abl(int(golden["abl_cells"]), zeta_half_mu)
+    row = int(golden["y_el_row"]) - 1
+    plan.set_criterion("l1_row", row)
+    plan.set_medium(torch.full((N, N), c0, dtype=torch.float32, device="cuda"), alpha0_db=0.0, y=1.5)
+    half = (int(golden["n_el"]) - 1) // 2
+    rows = np.arange(row - half, row + half + 1)
+    pos = np.stack([np.full(rows.size, golden["x_el_cells"] * dx), rows * dx], 1)
+    amp = np.full((1, rows.size), -1j * golden["source_strength"], dtype=np.complex64)
+    plan.set_source(pos, amp)
+    res = plan.solve(2000, golden["err_threshold"])
+    assert res.status == 0
+    n = int(res.n_terms[0])
+    lo = 0.9 * min(golden["iters_homog_gpu"], golden["iters_homog_cpu"])
+    hi = 1.1 * max(golden["iters_homog_gpu"], golden["iters_homog_cpu"])
+    assert lo <= n <= hi, n
+    # the beam has reached the far absorbing layer: the axial field 60 mm from the source is of the order of
+    # the field 10 mm from it (a lossless line source of width 10 mm, Rayleigh distance ~ 17 mm)
+    p = res.p[0]
+    near = float(p[row, int(golden["x_el_cells"]) + 500].abs())
+    far = float(p[row, int(golden["x_el_cells"]) + 3000].abs())
+    assert far > 0.2 * near

@@ -73,3 +73,46 @@ def test_cbs_first_terms_follow_the_definition():
     res = R.solve_cbs(V, S, g, eps, 1, 0.0)
     assert np.abs(res.p.reshape(n) - (u0 + u1)).max() < 1e-12 * np.abs(u0).max()
     assert abs(res.history[1] - np.linalg.norm(u1) / np.linalg.norm(u0 + u1)) < 1e-12
+
+
+# ---------------------------------------------------------------- paper mode
+def test_paper_mode_equals_algorithm_1_written_with_numpy_fft():
+    """Alg. 1 l.36-44 typed with numpy's FFT (a library routine, not the oracle's own):
+    periodic N-grid, window after every iteration, error of Eq. 30 on one row."""
+    N, f, c0 = 48, 1.0e6, 1500.0
+    dx = c0 / f / 6.0
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    rng = np.random.default_rng(3)
+    c = c0 * (1 + 0.02 * rng.standard_normal((N, N)))
+    V = R.potential(c, 0.0, 1.5, f, c0, 0.8)
+    S = np.zeros((N, N), complex)
+    S[20:28, 10] = -1.0e6j                       # Alg. 1 l.15: S = (0, -10^6) on the source pixels
+    g = R.green_spectrum((N, N), dx, k0, eps)
+    win = tuple(R.abl_window(N, 10) for _ in range(2))
+    A = win[1][:, None] * win[0][None, :]
+    res = R.solve_paper_mode(V, S, g, 25, 0.0, N // 2, windows=win)
+    psi = A * np.fft.ifft2(g * np.fft.fft2(S))
+    errs = []
+    for _ in range(25):
+        new = A * np.fft.ifft2(g * np.fft.fft2(V * psi + S))
+        errs.append(np.abs(new[N // 2] - psi[N // 2]).sum() / np.abs(psi[N // 2]).sum())
+        psi = new
+    assert np.abs(res.p - psi).max() < 1e-10 * np.abs(psi).max()
+    assert np.allclose(res.history[1:], errs, rtol=1e-9)
+
+
+def test_paper_mode_partial_sums_are_the_term_form_with_pad_factor_one():
+    """The Picard iterates on the periodic grid are the partial sums of the term form (Eq. 18 vs Eq. 19)."""
+    N, f, c0 = 32, 1.0e6, 1500.0
+    dx = c0 / f / 6.0
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    c = np.full((N, N), c0)
+    c[10:20, 12:22] = 1560.0
+    V = R.potential(c, 0.5, 1.1, f, c0, 0.8)
+    S = np.zeros((N, N), complex)
+    S[5, 8:24] = 1.0
+    g = R.green_spectrum((N, N), dx, k0, eps)
+    win = tuple(R.abl_window(N, 6) for _ in range(2))
+    a = R.solve_paper_mode(V, S, g, 12, 0.0, N // 2, windows=win)
+    b = R.solve(V, S, g, 12, 0.0, pad=1, windows=win)
+    assert np.abs(a.p - b.p).max() < 1e-12 * np.abs(b.p).max()
