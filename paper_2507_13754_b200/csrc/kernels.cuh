@@ -331,8 +331,8 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                         uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
                         pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
                     } else if (row == a.crit_row) {  // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row
-                        uu += sqrtf(fmaf(u.x, u.x, u.y * u.y));
-                        pp += sqrtf(fmaf(pold[it][j].x, pold[it][j].x, pold[it][j].y * pold[it][j].y));
+                        uu += hypotf(u.x, u.y);  // hypotf: no underflow of the squares for very small fields
+                        pp += hypotf(pold[it][j].x, pold[it][j].y);
                     }
                     x[j] = cmul(vpot[it][j], u);
                 }

@@ -101,3 +101,73 @@ def test_paper_homogeneous_case_reproduces_table_3_iteration_count(golden):
     near = float(p[row, int(golden["x_el_cells"]) + 500].abs())
     far = float(p[row, int(golden["x_el_cells"]) + 3000].abs())
     assert far > 0.2 * near
+
+
+def _paper_plan(golden, f, c, **medium):
+    from paper_2507_13754_b200.tbs import Plan
+    N, dx, c0 = int(golden["n_grid"]), golden["dx_m"], golden["v_f"]
+    plan = Plan((N, N), dx, [f], c0, golden["eps_over_k2"])
+    plan.set_boundary("periodic")
+    plan.set_abl(int(golden["abl_cells"]), golden["zeta_np_per_cm"] * (golden["abl_cells"] * dx * 100.0) / 2.0)
+    plan.set_criterion("l1_row", int(golden["y_el_row"]) - 1)
+    plan.set_medium(c, alpha0_db=0.0, y=1.5, **medium)
+    return plan
+
+
+def _paper_source(golden):
+    dx, row = golden["dx_m"], int(golden["y_el_row"]) - 1
+    half = (int(golden["n_el"]) - 1) // 2
+    rows = np.arange(row - half, row + half + 1)
+    pos = np.stack([np.full(rows.size, golden["x_el_cells"] * dx), rows * dx], 1)
+    return pos, np.full((1, rows.size), -1j * golden["source_strength"], dtype=np.complex64)
+
+
+def test_paper_scatterer_cases_follow_table_3(golden):
+    """PAPER.md:264 and Table 3: a disc of radius 50 dx on the axis, 40.2 mm from the line
+    source, v_s = 1350 / 1650 / 1800 m/s.  The paper's CPU code needs 162 / 155 / 164 iterations (its GPU column
+    prints 134 for all three); within 10 % here, and in the same order."""
+    from paper_2507_13754_b200.tbs import grid_harmonic_frequency
+    N, dx, c0 = int(golden["n_grid"]), golden["dx_m"], golden["v_f"]
+    f = grid_harmonic_frequency(int(golden["f_multiple"]), c0, N, dx)
+    row = int(golden["y_el_row"]) - 1
+    yy, xx = torch.meshgrid(torch.arange(N, device="cuda"), torch.arange(N, device="cuda"), indexing="ij")
+    xc = golden["x_el_cells"] + golden["scatterer_dist_m"] / dx
+    disc = (xx - xc) ** 2 + (yy - row) ** 2 < golden["scatterer_radius_cells"] ** 2
+    pos, amp = _paper_source(golden)
+    counts = {}
+    for vs in (1350, 1650, 1800):
+        c = torch.full((N, N), c0, dtype=torch.float32, device="cuda")
+        c[disc] = float(vs)
+        plan = _paper_plan(golden, f, c)
+        plan.set_source(pos, amp)
+        res = plan.solve(2000, golden["err_threshold"])
+        assert res.status == 0
+        counts[vs] = int(res.n_terms[0])
+        ref = golden[f"iters_vs{vs}_cpu"]
+        assert 0.9 * ref <= counts[vs] <= 1.1 * ref, (vs, counts[vs], ref)
+        del plan
+    assert counts[1650] < counts[1350] < counts[1800]
+
+
+def test_paper_nonlinear_case_follows_table_3_for_five_harmonics(golden):
+    """PAPER.md:266 and Table 3: fundamental and harmonics 2-5 of the homogeneous nonlinear
+    medium (B/A = 5), eps_h = 0.8 (h k_f)^2, solved one after the other.  The paper prints 135, 228, 306, 368,
+    416 iterations (CUDA) and 133, 225, 301, 362, 409 (CPU); each within 10 % here.  The fundamental is rescaled
+    to 1 MPa before the harmonic sources are formed (the counts do not depend on the amplitude; complex64 would
+    underflow at the paper's source strength by the fourth harmonic)."""
+    from paper_2507_13754_b200.tbs import grid_harmonic_frequency, solve_harmonics
+    N, dx, c0 = int(golden["n_grid"]), golden["dx_m"], golden["v_f"]
+    f1 = grid_harmonic_frequency(int(golden["f_multiple"]), c0, N, dx)
+    c = torch.full((N, N), c0, dtype=torch.float32, device="cuda")
+    plans = [_paper_plan(golden, h * f1, c, beta=1 + golden["b_over_a"] / 2, rho0=golden["rho_f"]) for h in range(1, 6)]
+    plans[0].set_source(*_paper_source(golden))
+    st, res = solve_harmonics(plans, 2000, golden["err_threshold"], int(golden["y_el_row"]) - 1, 1.0e6)
+    assert st == 0
+    counts = [int(r.n_terms[0]) for r in res]
+    for h, n in enumerate(counts, start=1):
+        lo = 0.9 * min(golden[f"iters_h{h}_gpu"], golden[f"iters_h{h}_cpu"])
+        hi = 1.1 * max(golden[f"iters_h{h}_gpu"], golden[f"iters_h{h}_cpu"])
+        assert lo <= n <= hi, (h, n)
+    # amplitudes fall from harmonic to harmonic
+    mags = [float(r.p[0].abs().max()) for r in res]
+    assert all(mags[i + 1] < mags[i] for i in range(4))
