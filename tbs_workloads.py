@@ -175,5 +175,26 @@ def cfg5(N: int = 256, nfreq: int = 1, seed: int = SEED0 + 5) -> Workload:
 CONFIGS = {1: cfg1, 2: cfg2, 3: cfg3, 4: cfg4, 5: cfg5}
 
 
+def paper_e1(N: int = 4096) -> Workload:
+    """The paper's own first experiment: N = 4096, dx = 0.02 mm, homogeneous lossless water,
+    f = the 55th harmonic of the periodic grid, 501-pixel line source of strength -i 10^6 along y at column
+    675, centred on row 2049 (1-based).  notes carries the paper-faithful solver options: periodic boundary,
+    450-cell layer with zeta mu/2 = 9.666, Eq. 30 on the centre row below 10^-5, cap 2000 iterations.  Smaller
+    N keep dx, the frequency, and scale the geometry."""
+    dx, c0 = 0.02e-3, 1500.0
+    f = 55 * c0 / (4096 * dx)
+    k = N / 4096.0
+    row = N // 2
+    half = int(round(250 * k))
+    rows = np.arange(row - half, row + half + 1)
+    pos = np.stack([np.full(rows.size, round(675 * k) * dx), rows * dx], 1).astype(np.float64)
+    amp = np.full((1, rows.size), -1.0e6j, dtype=np.complex64)
+    return Workload(name=f"paper_e1_2d_{N}_periodic", ndim=2, shape=(N, N), dx=dx, freqs=[f], c0=c0, rho0=1000.0,
+                    damping=0.8, alpha0_db=0.0, y=1.5, beta=3.5, c=np.full((N, N), c0, dtype=np.float32), rho=None,
+                    src_pos=pos, src_amp=amp, tol=1e-5, max_terms=2000,
+                    notes={"boundary": "periodic", "abl_cells": int(round(450 * k)), "zeta_half_mu": 9.666,
+                           "criterion_row": row})
+
+
 def make(idx: int, **kw) -> Workload:
     return CONFIGS[idx](**kw)
