@@ -146,7 +146,7 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
     return cudaErrorInvalidValue;
 }
 
-template <int N, bool FIRST, bool CBS>
+template <int N, bool FIRST, bool GEN>
 static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
     constexpr int TPL = tpl_of(N);
@@ -155,7 +155,7 @@ static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_att
     constexpr int ROWS = C::GROUPS * GR;
     constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
                             (FIRST ? 0 : (size_t)ROWS * N * sizeof(float4));
-    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, CBS>;
+    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN>;
     static int cap = 0;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -174,7 +174,8 @@ static cudaError_t launch_row_t(const RowArgs &a, cudaStream_t st, bool set_attr
         cudaError_t e = launch_row_tt<N, false, false>(a, st, true);
         return e != cudaSuccess ? e : launch_row_tt<N, false, true>(a, st, true);
     }
-    return a.ucbs ? launch_row_tt<N, false, true>(a, st, false) : launch_row_tt<N, false, false>(a, st, false);
+    return (a.ucbs || a.crit_row >= 0) ? launch_row_tt<N, false, true>(a, st, false)
+                                        : launch_row_tt<N, false, false>(a, st, false);
 }
 
 template <bool FIRST>

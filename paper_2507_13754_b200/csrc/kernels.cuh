@@ -196,11 +196,13 @@ struct RowArgs {
 //
 // FIRST = true : forward half only, w = src * src_scale (term 0: u_0 = G S, Eq. 20)
 // FIRST = false: inverse half (K3) + forward half (K1) of the next term
-// CBS   = true : the term update of the convergent Born series instead of u = A G(V u)
+// GEN   = true : the general variant: the convergent Born series update (a.ucbs) and/or
+//                the one-row L1 criterion of Eq. 30 (a.crit_row >= 0), chosen at run time; GEN = false is
+//                the hot path (traditional series, full-grid L2 measure) without either
 // Persistent and group-independent: group G of CTA B walks row tiles (B*GROUPS + G) + i*gridDim.x*
 // GROUPS; the W rows of its next tile arrive by one bulk copy (completion on the group's mbarrier)
 // in a staging buffer while the current tile computes.
-template <int N, int GROUPS, int MINB, bool FIRST, bool CBS>
+template <int N, int GROUPS, int MINB, bool FIRST, bool GEN>
 __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
@@ -259,7 +261,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             for (int i = gl; i < GR * N / 16; i += GT) {
                 prefetch_l2(a.p + (long long)gt * GR * N + i * 16);
                 prefetch_l2(a.V + (long long)gt * GR * N + i * 16);
-                if (CBS) prefetch_l2(a.ucbs + (long long)gt * GR * N + i * 16);
+                if (GEN && a.ucbs) prefetch_l2(a.ucbs + (long long)gt * GR * N + i * 16);
             }
             wrow *= __ldg(&a.ay[row % a.ny]);
             if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
@@ -318,7 +320,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     const long long gi = (long long)row * N + pos;
                     const float wgt = wrow * __ldg(&a.ax[pos]);
                     float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
-                    if (CBS) {
+                    if (GEN && a.ucbs) {
                         // convergent Born series: u_{n+1} = u_n + gamma (A G(V u_n) - u_n), gamma = i V / eps
                         const float2 gam = make_float2(-vpot[it][j].y * a.inv_e, vpot[it][j].x * a.inv_e);
                         const float2 uo = term > 0 ? a.ucbs[gi] : make_float2(0.f, 0.f);
@@ -327,7 +329,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                     }
                     const float2 pv = cadd(pold[it][j], u);
                     a.p[gi] = pv;
-                    if (a.crit_row < 0) {
+                    if (!GEN || a.crit_row < 0) {
                         uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
                         pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
                     } else if (row == a.crit_row) {  // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row
@@ -395,7 +397,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
                 __threadfence();
                 const double nu = *((volatile double *)&a.norms[2 * term]);
                 const double np = *((volatile double *)&a.norms[2 * term + 1]);
-                const double r = a.crit_row < 0 ? sqrt(nu) / sqrt(np) : (term == 0 ? 1.0 : nu / np);
+                const double r = (!GEN || a.crit_row < 0) ? sqrt(nu) / sqrt(np) : (term == 0 ? 1.0 : nu / np);
                 a.history[term] = (term == 0) ? 1.0 : r;
                 a.ctl->ticket = 0;
                 a.ctl->next_tile = 0;
