@@ -63,6 +63,15 @@ size_t tbs_plan_workspace_bytes(const tbs_plan *plan);
 /* Text of the last error on this plan (plan-owned storage, valid until the next call). */
 const char *tbs_last_error(const tbs_plan *plan);
 
+/* Homogeneous absorbing(-dispersive) medium in the paper's own form, Eq. 24: the potential
+ * acts in k-space, VV(k) = -i tau w k^nu + eta k^(nu+1) - i eps with tau = -2 alpha0 v_f^(nu-1),
+ * eta = 2 alpha0 v_f^nu tan(pi nu/2), v_f = the plan's c0, alpha0_si in Np (rad/s)^-nu m^-1;
+ * dispersive = 0 drops the eta term (the "absorbing" row of Table 3).  The term update becomes
+ * u_{n+1} = A F^-1[ghat(p) VV(|p|) F[u_n]]: the spatial potential is ignored (tbs_set_medium not needed)
+ * and the multiplier is applied inside the fused Green's-spectrum stage.  alpha0_si = 0 switches back to the
+ * spatial potential, which then has to be set again.  Not combined with TBS_SCHEME_CBS. */
+tbs_status tbs_set_kspace_absorption(tbs_plan *plan, double alpha0_si, double nu, int dispersive);
+
 /* Boundary treatment (default TBS_BOUNDARY_PAD: zero-pad to 2N per axis, linear convolution, crop --
  * BASELINE north_star).  TBS_BOUNDARY_PERIODIC is the paper's own: the FFTs act on the N-grid itself
  * (Eq. 19, Alg. 1 l.36-38) and wrap-around is left to the absorbing layer of tbs_set_abl

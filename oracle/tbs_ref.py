@@ -272,3 +272,57 @@ def solve_paper_mode(V, S, ghat_periodic, max_iter: int, tol: float, row: int, w
             status = OK
             break
     return RefResult(status, psi, np.array(hist), l, u if max_iter > 0 else psi)
+
+
+def kspace_potential(shape_padded, dx: float, alpha0_si: float, nu: float, f_hz: float, c0: float, damping: float,
+                     dispersive: bool = True):
+    """VV(k) = -i tau w k^nu + eta k^(nu+1) - i eps on the FFT grid (Eq. 24; Alg. 1 l.23,
+    PAPER.md:323), tau = -2 alpha0 v_f^(nu-1), eta = 2 alpha0 v_f^nu tan(pi nu/2), k = |p|."""
+    w = 2.0 * math.pi * f_hz
+    k0, eps = wavenumber(f_hz, c0, damping)
+    tau = -2.0 * alpha0_si * c0 ** (nu - 1.0)
+    eta = 2.0 * alpha0_si * c0 ** nu * math.tan(math.pi * nu / 2.0) if dispersive else 0.0
+    k2 = np.zeros(shape_padded)
+    nd = len(shape_padded)
+    for ax, m in enumerate(shape_padded):
+        p = 2.0 * math.pi * np.fft.fftfreq(m, d=dx)
+        shp = [1] * nd
+        shp[ax] = m
+        k2 = k2 + (p ** 2).reshape(shp)
+    k = np.sqrt(k2)
+    return -1j * tau * w * k ** nu + eta * k ** (nu + 1.0) - 1j * eps
+
+
+def solve_kspace(S, ghat, VV, max_terms: int, tol: float, pad: int = 2, windows=None, row=None) -> RefResult:
+    """Eq. 24 in term form: u_0 = A G S, u_{n+1} = A F^-1[ghat VV F[u_n]], p = sum u_n (the Picard iterates of
+    Eq. 24 are these partial sums).  row = None: r_n = ||u_n||_2/||p_n||_2; row = r: Eq. 30 on that row."""
+    S = np.ascontiguousarray(S, dtype=np.complex128)
+    A = np.ones(S.shape)
+    if windows is not None:
+        nd = S.ndim
+        for a in range(nd):
+            shp = [1] * nd
+            shp[nd - 1 - a] = -1
+            A = A * np.asarray(windows[a], dtype=np.float64).reshape(shp)
+    nx = S.shape[-1]
+    gv = np.ascontiguousarray(ghat * VV)
+    u = A * apply_G(S, ghat, pad)
+    p = u.copy()
+    hist = [1.0]
+    status, k = NOT_CONVERGED, 0
+    for k in range(1, max_terms + 1):
+        u = A * apply_G(u, gv, pad)
+        if row is None:
+            p += u
+            r = math.sqrt(float(np.vdot(u, u).real)) / math.sqrt(float(np.vdot(p, p).real))
+        else:
+            r = float(np.abs(u.reshape(-1, nx)[row]).sum() / np.abs(p.reshape(-1, nx)[row]).sum())
+            p += u
+        hist.append(r)
+        if not math.isfinite(r):
+            status = ERR_DIVERGED
+            break
+        if r < tol:
+            status = OK
+            break
+    return RefResult(status, p, np.array(hist), k, u)

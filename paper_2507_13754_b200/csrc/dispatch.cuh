@@ -91,12 +91,12 @@ static inline cudaError_t make_conv_tensor_map(CUtensorMap *out, const void *bas
 }
 static inline int conv_tile_width(int N);
 
-template <int N>
-static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr) {
+template <int N, bool KABS>
+static cudaError_t launch_conv_tt(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr) {
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = T * tpl_of(N);
     constexpr size_t smem = (size_t)conv_smem_bytes(N, T);
-    auto kern = k_conv<N, T, ConvCfg<N>::MINB>;
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB, KABS>;
     static int cap = 0;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -108,6 +108,16 @@ static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int 
     const long long total = (long long)n_outer * (a.inner_len / T);
     kern<<<(unsigned)(total < cap ? total : cap), NT, smem, st>>>(b, *tmap);
     return cudaGetLastError();
+}
+
+template <int N>
+static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr) {
+    if (set_attr) {
+        cudaError_t e = launch_conv_tt<N, false>(a, tmap, n_outer, st, true);
+        return e != cudaSuccess ? e : launch_conv_tt<N, true>(a, tmap, n_outer, st, true);
+    }
+    return a.kabs.nu > 0.f ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false)
+                           : launch_conv_tt<N, false>(a, tmap, n_outer, st, false);
 }
 
 static cudaError_t launch_conv(int N, const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st,

@@ -215,9 +215,17 @@ __device__ __forceinline__ void load_p2x2(float2 (&pp)[RL], const float2 *__rest
 #pragma unroll
     for (int j = 0; j < RL; ++j) pp[j] = TSM ? p2x2[j * (N / RL) + b] : __ldg(p2x2 + j * (N / RL) + b);
 }
-template <int N, int RL, class Lay, bool TSM = false>
+// Parameters of the k-space multiplier potential of Eq. 24, non-dimensional:
+//   VV(k)/k0^2 = -i A kappa^nu + B kappa^(nu+1) - i e,  kappa = k/k0,  A = tau w k0^(nu-2),  B = eta k0^(nu-1).
+struct KAbs {
+    float A, B, nu, e;
+};
+
+// KABS = true: the spectrum of the (unmultiplied) term is multiplied by ghat(p) VV(|p|) instead of ghat(p)
+// (homogeneous absorbing-dispersive medium, Eq. 24); kappa^2 = 1 + e alpha comes from the same tables.
+template <int N, int RL, class Lay, bool TSM = false, bool KABS = false>
 __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
-                                               float a_line) {
+                                               float a_line, KAbs ka = KAbs{0.f, 0.f, 0.f, 0.f}) {
     const int base = b * RL;
     float2 pp[RL];
     load_p2x2<N, RL, TSM>(pp, p2x2, b);
@@ -232,7 +240,20 @@ __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, cons
         const float2 al = __fadd2_rn(pp[k], f2(a_line));
         const float2 d = __ffma2_rn(al, al, f2(1.0f));
         const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
-        u[k] = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};
+        P2 w = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};
+        if (KABS && ka.nu > 0.f) {
+            // kappa^nu = exp2(nu/2 log2(kappa^2)); frequencies masked for the periodic boundary (alpha ~ 1e18) give 0
+            float2 q = __ffma2_rn(al, f2(ka.e), f2(1.0f));  // kappa^2 = |p|^2/k0^2 (>= 0 up to rounding)
+            q = make_float2(fmaxf(q.x, 0.f), fmaxf(q.y, 0.f));
+            const float2 lg = make_float2(__log2f(q.x), __log2f(q.y));
+            const float2 kn = make_float2(exp2f(0.5f * ka.nu * lg.x), exp2f(0.5f * ka.nu * lg.y));
+            const float2 k1 = make_float2(exp2f(0.5f * lg.x), exp2f(0.5f * lg.y));
+            const float2 ok = make_float2(al.x < 1.0e17f ? 1.f : 0.f, al.y < 1.0e17f ? 1.f : 0.f);
+            const float2 vr = __fmul2_rn(__fmul2_rn(__fmul2_rn(kn, k1), f2(ka.B)), ok);                    // Re VV/k0^2
+            const float2 vi = __fmul2_rn(neg2(__ffma2_rn(kn, f2(ka.A), f2(ka.e))), ok);                    // Im VV/k0^2
+            w = P2{__ffma2_rn(w.re, vr, neg2(__fmul2_rn(w.im, vi))), __ffma2_rn(w.re, vi, __fmul2_rn(w.im, vr))};
+        }
+        u[k] = w;
     }
     pbfly<RL, +1>(u);
 #pragma unroll

@@ -43,6 +43,7 @@ struct ColArgs {
     const float *p2_inner;  // [inner_len] of the inner (x) axis, position order  (CONV)
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
     float inv_e;            // k0^2/eps = 1/damping
+    KAbs kabs;              // k-space multiplier potential of Eq. 24 (k_conv<..., KABS = true> only)
     Luts lut;
     const Ctl *ctl;
 };
@@ -420,7 +421,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
 // tile buffer used in place for both directions; the last inverse stage of a tile is fused with the
 // first forward stage of the next one (as in k_row), so a tile costs four stages and ONE CTA-wide
 // barrier; between them the T line groups run on their own barriers.
-template <int N, int T, int MINB>
+template <int N, int T, int MINB, bool KABS>
 __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
@@ -524,8 +525,10 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
             if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
             a_line *= a.inv_e;
+            KAbs ka = a.kabs;
+            if (KABS && a.ctl->term == 0) ka.nu = 0.f;  // term 0 is u_0 = A G S: the plain Green's spectrum
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM>(wk, line, b, p2_tab, a_line);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line, ka);
             group_sync<GT>(g);
         }
         if (R2 > 0) {

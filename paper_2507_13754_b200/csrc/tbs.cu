@@ -29,6 +29,7 @@ struct Freq {
     cudaGraphExec_t graph = nullptr;
     int graph_batch = 0;
     bool have_V = false, have_S = false;
+    KAbs kabs = {0.f, 0.f, 0.f, 0.f};  // nu > 0: k-space multiplier potential of Eq. 24 instead of V(r)
 };
 
 }  // namespace
@@ -127,6 +128,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     memset(&a, 0, sizeof a);
     a.ctl = f.ctl;
     a.inv_e = (float)(1.0 / pl->damping);
+    a.kabs = f.kabs;
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
@@ -339,6 +341,36 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
         return st;
     }
     *out = pl;
+    return TBS_OK;
+}
+
+__global__ void k_fill_complex(float2 *dst, float2 v, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = v;
+}
+
+tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, int dispersive) {
+    if (!pl || !(alpha0_si >= 0.0)) return TBS_ERR_INVALID_ARG;
+    if (alpha0_si > 0.0 && (!(nu > 0.0) || nu > 2.0 || fabs(nu - 1.0) < 1e-9))
+        return fail(pl, TBS_ERR_INVALID_ARG, "power-law exponent must lie in (0, 2] and differ from 1 (PAPER.md:53)");
+    for (auto &f : pl->fr) {
+        if (alpha0_si == 0.0) {
+            f.kabs = KAbs{0.f, 0.f, 0.f, 0.f};
+            f.have_V = false;  // the spatial potential has to be set again
+            continue;
+        }
+        // tau = -2 alpha0 v_f^(nu-1), eta = 2 alpha0 v_f^nu tan(pi nu/2)
+        const double tau = -2.0 * alpha0_si * pow(pl->c0, nu - 1.0);
+        const double eta = dispersive ? 2.0 * alpha0_si * pow(pl->c0, nu) * tan(kPi * nu / 2.0) : 0.0;
+        f.kabs.A = (float)(tau * f.omega * pow(f.k0, nu - 2.0));
+        f.kabs.B = (float)(eta * pow(f.k0, nu - 1.0));
+        f.kabs.nu = (float)nu;
+        f.kabs.e = (float)pl->damping;
+        k_fill_complex<<<nblk(pl->npts, 256), 256>>>(f.V, make_float2(1.f, 0.f), pl->npts);  // the term passes unmultiplied
+        f.have_V = true;
+    }
+    destroy_graphs(pl);
+    CU(pl, cudaDeviceSynchronize());
     return TBS_OK;
 }
 

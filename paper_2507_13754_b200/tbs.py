@@ -105,6 +105,10 @@ class Plan:
         code = {"born": 0, "tbs": 0, "cbs": 1}[scheme] if isinstance(scheme, str) else int(scheme)
         self._check(self._L.tbs_set_scheme(self._h, code))
 
+    def set_kspace_absorption(self, alpha0_si, nu, dispersive=True):
+        """tbs_set_kspace_absorption: homogeneous power-law medium as the k-space multiplier of Eq. 24."""
+        self._check(self._L.tbs_set_kspace_absorption(self._h, float(alpha0_si), float(nu), int(bool(dispersive))))
+
     def set_boundary(self, boundary):
         """tbs_set_boundary: "pad" (zero-pad/crop, default) or "periodic" (the paper's N-grid FFTs)."""
         code = {"pad": 0, "periodic": 1}[boundary] if isinstance(boundary, str) else int(boundary)

@@ -204,3 +204,54 @@ def test_paper_absorbing_dispersive_case_count_and_attenuation_law(golden):
     d1, d2 = int(10e-3 / dx), int(50e-3 / dx)
     measured = (fields[1][col0 + d2] / fields[0][col0 + d2]) / (fields[1][col0 + d1] / fields[0][col0 + d1])
     assert abs(measured / np.exp(-alpha * (d2 - d1) * dx) - 1) < 0.02, measured
+
+
+@pytest.mark.parametrize("boundary", ["pad", "periodic"])
+def test_kspace_multiplier_potential_matches_oracle(boundary):
+    """Eq. 24 through tbs_set_kspace_absorption, against the oracle's solve_kspace."""
+    from paper_2507_13754_b200.tbs import Plan
+    N, f, c0 = 128, 1.0e6, 1500.0
+    dx = c0 / f / 8.0
+    a0, nu, abl = 4.0e-9, 1.5, 16
+    rows = np.arange(N // 2 - 12, N // 2 + 13)
+    pos = np.stack([np.full(rows.size, (abl + 5) * dx), rows * dx], 1)
+    amp = np.full((1, rows.size), -1.0e6j, dtype=np.complex64)
+    pad = 1 if boundary == "periodic" else 2
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    g = R.green_spectrum((pad * N, pad * N), dx, k0, eps)
+    VV = R.kspace_potential((pad * N, pad * N), dx, a0, nu, f, c0, 0.8)
+    S = R.deposit((N, N), dx, pos, amp[0])
+    win = tuple(R.abl_window(N, abl) for _ in range(2))
+    ref = R.solve_kspace(S, g, VV, 3000, 1e-6, pad=pad, windows=win)
+    plan = Plan((N, N), dx, [f], c0, 0.8)
+    plan.set_boundary(boundary)
+    plan.set_abl(abl, 9.666)
+    plan.set_kspace_absorption(a0, nu)
+    plan.set_source(pos, amp)
+    res = plan.solve(3000, 1e-6)
+    assert res.status == 0 and ref.status == R.OK
+    assert abs(int(res.n_terms[0]) - ref.n_terms) <= 1
+    compare_fields(res.p[0].cpu().numpy(), ref.p, f"Eq. 24, {boundary}")
+    compare_history(res.history[0], ref.history, min(int(res.n_terms[0]), ref.n_terms))
+
+
+def test_paper_absorbing_rows_of_table_3_with_the_kspace_multiplier(golden):
+    """Table 3 in the paper's own formulation (Eq. 24): "absorbing" (lossy operator only)
+    133 / 134 iterations, "absorbing-dispersive" 132 / 131; within 10 % here."""
+    from paper_2507_13754_b200.tbs import Plan, grid_harmonic_frequency
+    N, dx, c0 = int(golden["n_grid"]), golden["dx_m"], golden["v_f"]
+    f = grid_harmonic_frequency(int(golden["f_multiple"]), c0, N, dx)
+    for dispersive, key in ((False, "abs"), (True, "absdisp")):
+        plan = Plan((N, N), dx, [f], c0, golden["eps_over_k2"])
+        plan.set_boundary("periodic")
+        plan.set_abl(int(golden["abl_cells"]), golden["zeta_np_per_cm"] * (golden["abl_cells"] * dx * 100.0) / 2.0)
+        plan.set_criterion("l1_row", int(golden["y_el_row"]) - 1)
+        plan.set_kspace_absorption(golden["alpha0_si"], golden["nu"], dispersive)
+        plan.set_source(*_paper_source(golden))
+        res = plan.solve(2000, golden["err_threshold"])
+        assert res.status == 0
+        n = int(res.n_terms[0])
+        lo = 0.9 * min(golden[f"iters_{key}_gpu"], golden[f"iters_{key}_cpu"])
+        hi = 1.1 * max(golden[f"iters_{key}_gpu"], golden[f"iters_{key}_cpu"])
+        assert lo <= n <= hi, (key, n)
+        del plan

@@ -116,3 +116,84 @@ def test_paper_mode_partial_sums_are_the_term_form_with_pad_factor_one():
     a = R.solve_paper_mode(V, S, g, 12, 0.0, N // 2, windows=win)
     b = R.solve(V, S, g, 12, 0.0, pad=1, windows=win)
     assert np.abs(a.p - b.p).max() < 1e-12 * np.abs(b.p).max()
+
+
+# ---------------------------------------------------------------- k-space multiplier potential (Eq. 24)
+def _kspace_case(ny, nx, ppw=8.0):
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / ppw
+    return f, c0, dx
+
+
+def test_kspace_potential_on_shell_value_and_printed_constants(golden):
+    """VV(k_f) + i eps = k_f^nu (eta k_f - i tau w) = 2 k_f alpha (tan(pi nu/2) + i), alpha = alpha0 w^nu (Eq. 3,
+    PAPER.md:51): the multiplier reproduces the power law on shell; tau, eta as printed in Table 4."""
+    f, c0 = golden["f_hz"], golden["v_f"]
+    a0, nu = golden["alpha0_si"], golden["nu"]
+    w = 2 * np.pi * f
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    M = 64
+    dx = 2 * np.pi / (M * k0) * 8          # so that bin 8 of the FFT grid sits exactly on |p| = k0
+    VV = R.kspace_potential((M,), dx, a0, nu, f, c0, 0.8)
+    on_shell = VV[8] + 1j * eps
+    alpha = a0 * w ** nu
+    expect = 2 * k0 * alpha * (np.tan(np.pi * nu / 2) + 1j)
+    assert abs(on_shell - expect) < 1e-9 * abs(expect)
+    tau = -2 * a0 * c0 ** (nu - 1)
+    eta = 2 * a0 * c0 ** nu * np.tan(np.pi * nu / 2)
+    assert abs(tau / golden["tau"] - 1) < 0.02 and abs(eta / golden["eta"] - 1) < 0.02
+
+
+def test_kspace_series_equals_equation_24_typed_with_numpy_fft():
+    f, c0, dx = _kspace_case(32, 32)
+    N = 40
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    a0, nu = 8.0e-9, 1.5
+    g = R.green_spectrum((N, N), dx, k0, eps)
+    VV = R.kspace_potential((N, N), dx, a0, nu, f, c0, 0.8)
+    S = np.zeros((N, N), complex)
+    S[14:26, 8] = -1.0e6j
+    win = tuple(R.abl_window(N, 8) for _ in range(2))
+    A = win[1][:, None] * win[0][None, :]
+    res = R.solve_kspace(S, g, VV, 20, 0.0, pad=1, windows=win, row=N // 2)
+    psi = A * np.fft.ifft2(g * np.fft.fft2(S))
+    errs = []
+    for _ in range(20):                     # Eq. 24 as printed, Picard form, window after every iteration
+        new = A * np.fft.ifft2(g * (VV * np.fft.fft2(psi) + np.fft.fft2(S)))
+        errs.append(np.abs(new[N // 2] - psi[N // 2]).sum() / np.abs(psi[N // 2]).sum())
+        psi = new
+    assert np.abs(res.p - psi).max() < 1e-10 * np.abs(psi).max()
+    assert np.allclose(res.history[1:], errs, rtol=1e-8)
+
+
+def test_kspace_series_plane_wave_decays_with_the_power_law():
+    """A source uniform in y on a grid periodic in y radiates plane waves along x; between two planes their
+    amplitude and phase must follow the complex wavenumber of the absorbing-dispersive wave equation (Eq. 7)."""
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / 8.0
+    ny, nx = 4, 1024
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    a0, nu = 6.0e-9, 1.5                      # alpha = a0 w^nu ~ 94 Np/m: e^-1 over ~57 cells
+    g = R.green_spectrum((ny, nx), dx, k0, eps)
+    VV = R.kspace_potential((ny, nx), dx, a0, nu, f, c0, 0.8)
+    S = np.zeros((ny, nx), complex)
+    S[:, 200] = 1.0
+    win = (R.abl_window(nx, 150), np.ones(ny))
+    res = R.solve_kspace(S, g, VV, 3000, 1e-10, pad=1, windows=win)
+    assert res.status == R.OK
+    a, b = 300, 700
+    # plane wave e^{iKx} in Eq. 7 (PAPER.md:72): K^2 = k_f^2 - i tau w K^nu + eta K^(nu+1); to first order in
+    # alpha/k this is K = k_f + alpha (tan(pi nu/2) + i) with alpha = alpha0 w^nu (Eq. 3), solved exactly here
+    w = 2 * np.pi * f
+    tau = -2 * a0 * c0 ** (nu - 1)
+    eta = 2 * a0 * c0 ** nu * np.tan(np.pi * nu / 2)
+    K = complex(k0)
+    for _ in range(200):
+        K = np.sqrt(k0 ** 2 - 1j * tau * w * K ** nu + eta * K ** (nu + 1))
+    alpha = a0 * w ** nu
+    assert abs(K - (k0 + alpha * (np.tan(np.pi * nu / 2) + 1j))) < 0.1 * alpha      # the first-order form
+    ratio = abs(res.p[0, b]) / abs(res.p[0, a])
+    assert abs(ratio / np.exp(-K.imag * (b - a) * dx) - 1) < 0.01, ratio
+    dphi = np.unwrap(np.angle(res.p[0, a:b + 1]))
+    Kre = (dphi[-1] - dphi[0]) / ((b - a) * dx)
+    assert abs(Kre / K.real - 1) < 1e-3
