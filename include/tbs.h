@@ -132,7 +132,12 @@ tbs_status tbs_set_source_field(tbs_plan *plan, int ifreq, const float *S, void 
  *   p_out [nfreq][n][2]: dev (tbs_solve) or host (tbs_solve_host) complex64 field.
  *   history [nfreq][max_terms+1] host doubles: history[k] = ||u_k||_2/||p_k||_2, history[0] = 1;
  *     entries after n_terms are 0.   n_terms [nfreq] host: index of the last term added.
- * Synchronises `stream` before returning.  Returns the worst status over frequencies. */
+ * Synchronises `stream` before returning.  Returns the worst status over frequencies.
+ * Range: fields and norms are complex64 / fp32 partial sums; |u_n|^2 must stay inside the fp32 range, i.e.
+ * term magnitudes between about 1e-19 and 1e19.  A series whose terms fall below that (harmonics 3-5 of a
+ * source of arbitrary small strength) reports TBS_ERR_DIVERGED (0/0); scale the source, or use the
+ * surface-pressure rescaling of tbs_solve_harmonics.  The Eq. 30 row criterion uses hypotf and has the
+ * full fp32 range. */
 tbs_status tbs_solve(tbs_plan *plan, int max_terms, double tol, float *p_out, double *history,
                      int32_t *n_terms, void *stream);
 tbs_status tbs_solve_host(tbs_plan *plan, int max_terms, double tol, float *p_out_host,
