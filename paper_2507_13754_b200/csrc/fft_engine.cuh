@@ -6,7 +6,9 @@
 // out), so no reorder pass ever runs: the Green's spectrum ghat(p) is even in every
 // component of p and is simply indexed in the scrambled order (tables are built in "position
 // order" on the host).  Data lives in shared memory between stages; every stage reads and writes
-// the same positions ("in place"), so one __syncthreads() separates two stages.
+// the same positions ("in place"), so one barrier of the threads that own the line separates two
+// stages.  This file holds the scalar form (k_col) and what both forms share; fft_engine_x2.cuh holds
+// the packed form (k_row, k_conv).
 //
 // Zero padding N -> M = 2N (BASELINE.json north_star) is never materialised:
 //   X[2k+s] = sum_{j<N} (x[j] w_M^{js}) w_N^{jk}            (forward, s = 0, 1: two length-N FFTs)
@@ -17,8 +19,6 @@
 #include <stdint.h>
 
 namespace tbs {
-
-constexpr int NTW = 8192;  // twiddle table length: tw[k] = exp(-2 pi i k / NTW)
 
 // ---- complex helpers -------------------------------------------------------------------------
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -70,9 +70,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
 __device__ __forceinline__ void cp_async16(void *dst, const void *src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_async8(void *dst, const void *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -88,7 +85,6 @@ template <> struct Radix<1024> { static constexpr int R1 = 8,  R2 = 8,  RL = 16;
 template <> struct Radix<2048> { static constexpr int R1 = 8,  R2 = 16, RL = 16; };
 template <> struct Radix<4096> { static constexpr int R1 = 16, R2 = 16, RL = 16; };
 
-__host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
 // bit reversal of i within log2(R) bits
 __host__ __device__ constexpr int brev(int i, int R) {
     int r = 0;
@@ -196,16 +192,6 @@ struct ColLay {
     template <int NBL>
     __device__ static __forceinline__ void split(int w, int &line, int &b) { line = w % T_; b = w / T_; }
 };
-// Row tile: each line contiguous, one pad slot per 16 positions, PAD extra slots per line (PAD = 4
-// makes a cooperative read across 4 lines x 4 positions conflict-free for N >= 256).
-template <int N, int PAD = 0>
-struct RowLay {
-    static constexpr int PITCH = N + N / 16 + PAD;
-    __device__ static __forceinline__ int addr(int line, int pos) { return line * PITCH + pos + (pos >> 4); }
-    template <int NBL>
-    __device__ static __forceinline__ void split(int w, int &line, int &b) { b = w % NBL; line = w / NBL; }
-};
-
 // Threads that own one line in the line-group kernels (k_row, k_conv): one radix-16 item each in
 // the widest stage.  Groups of TPL >= 32 threads synchronise on a named barrier of their own,
 // smaller groups share a warp and use __syncwarp, so no stage waits for the whole CTA.

@@ -5,12 +5,14 @@
 //                         partial ||u||^2, ||p||^2 -> last CTA finalises r_n and the stop flag
 //          forward half:  w = V.u (or the source S for term 0) -> zero-pad -> FFT_x -> W row
 //          u never leaves the chip between the two halves (cross-term fusion).
-//   k_col<MODE>: per tile of T adjacent lines along a strided axis (y in 2-D; y and z in 3-D).
-//          CONV: pad, FFT, .ghat, IFFT, crop, in place   (K2 in 2-D, the z pass in 3-D)
-//          FWD : pad, FFT  N -> 2N positions             (3-D y pass, forward)
-//          INV : IFFT, crop  2N positions -> N           (3-D y pass, inverse)
+//   k_conv: per tile of T adjacent lines along a strided axis (y in 2-D, z in 3-D): pad, FFT, .ghat,
+//          IFFT, crop, in place (K2 in 2-D, the z pass in 3-D); tiles move by TMA.
+//   k_col<MODE> (3-D y passes, scalar engine):
+//          FWD : pad, FFT  N -> 2N positions
+//          INV : IFFT, crop  2N positions -> N
 // Both parity halves of a padded line (fft_engine.cuh) are resident in shared memory at once, so
-// the input is read once and the twiddles of a butterfly pair are fetched once.
+// the input is read once and the twiddles of a butterfly pair are fetched once.  k_row and k_conv
+// use the packed engine of fft_engine_x2.cuh (both halves in one register pair).
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime, tbs.cu)
 
@@ -48,9 +50,9 @@ struct ColArgs {
     const Ctl *ctl;
 };
 
-// Persistent: each CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...  For CONV and FWD the N
-// input positions of the next tile are fetched with cp.async into a staging buffer while the
-// current tile computes.
+// Persistent: each CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...  For FWD the N input
+// positions of the next tile are fetched with cp.async into a staging buffer while the current
+// tile computes.
 template <int N, int T, int NT, int MODE>
 __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     using P = Radix<N>;
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     constexpr int HALF = N * T;
     using Lay = ColLay<N, T, RL>;
     extern __shared__ __align__(1024) float2 sm[];
-    float2 *stg = sm + 2 * HALF;  // [N][T] staged input tile (CONV, FWD)
+    float2 *stg = sm + 2 * HALF;  // [N][T] staged input tile (FWD)
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
