@@ -24,8 +24,12 @@
  * Hankel / spherical closed forms (P2), lossless line-source Hankel sum with ABL (P3),
  * exact diagonal special case (P4), brute-force first term (P5), dense Lippmann-Schwinger
  * solve (P6), invariants (P7), FFT vs naive DFT (P8).
- * parity unpinned: the paper's Table 3 iteration counts and its k-Wave agreement figures
- * -- they belong to the periodic+ABL variant and need k-Wave.
+ * The Python side (tbs_ref.py) adds, on top of apply_G: the harmonic sources of Eqs. 28b-28e (pinned by
+ * a Westervelt sum-frequency projection), the convergent Born series, Algorithm 1 as printed (periodic
+ * grid, Eq. 30) and the k-space multiplier potential of Eq. 24 (tests/test_oracle_pins_d.py).
+ * parity unpinned: the paper's k-Wave agreement figures (they need k-Wave).  The iteration
+ * counts of Table 3 are checked on the GPU path, whole table within 7 %
+ * (tests/test_gpu_paper_mode.py); the oracle itself is not run at 4096^2.
  */
 #include <complex.h>
 #include <math.h>
