@@ -136,8 +136,8 @@ tbs_status tbs_set_source_field(tbs_plan *plan, int ifreq, const float *S, void 
  * Range: fields and norms are complex64 / fp32 partial sums; |u_n|^2 must stay inside the fp32 range, i.e.
  * term magnitudes between about 1e-19 and 1e19.  A series whose terms fall below that (harmonics 3-5 of a
  * source of arbitrary small strength) reports TBS_ERR_DIVERGED (0/0); scale the source, or use the
- * surface-pressure rescaling of tbs_solve_harmonics.  The Eq. 30 row criterion uses hypotf and has the
- * full fp32 range. */
+ * surface-pressure rescaling of tbs_solve_harmonics.  The Eq. 30 row criterion pre-scales by 2^20 and
+ * covers 1e-25 < |u_n| < 1e13. */
 tbs_status tbs_solve(tbs_plan *plan, int max_terms, double tol, float *p_out, double *history,
                      int32_t *n_terms, void *stream);
 tbs_status tbs_solve_host(tbs_plan *plan, int max_terms, double tol, float *p_out_host,

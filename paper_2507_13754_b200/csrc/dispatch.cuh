@@ -15,11 +15,11 @@ template <> struct ColCfg<512>  { static constexpr int T = 8,  NT = 512; };
 
 // Row kernel k_row: GROUPS independent line groups per CTA (a group = N/16 threads on one row, or
 // one warp on 32/(N/16) rows), at least MINB CTAs per SM (register cap).  Shared memory per row =
-// N*16 bytes of work area + N*16 bytes of W staging.  Values measured on B200 (cfg2-cfg5).
+// N*16 bytes of work area + N*16 bytes of W staging (N = 4096: no staging, two items per thread).  Values measured on B200 (cfg2-cfg5).
 template <int N> struct RowCfg { static constexpr int GROUPS = 4, MINB = 2; };   // N <= 512
 template <> struct RowCfg<1024> { static constexpr int GROUPS = 2, MINB = 3; };
 template <> struct RowCfg<2048> { static constexpr int GROUPS = 1, MINB = 3; };
-template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 1; };
+template <> struct RowCfg<4096> { static constexpr int GROUPS = 1, MINB = 2; };
 
 // Convolution kernel k_conv: T adjacent lines per CTA, T * max(N/16, 4) threads, at least MINB CTAs
 // per SM.  Shared memory = T*N*16 bytes of work area + N*T*8 bytes of input staging (+ tables).
@@ -159,12 +159,12 @@ static cudaError_t launch_col(int N, const ColArgs &a, int n_outer, cudaStream_t
 template <int N, bool FIRST, bool GEN>
 static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr) {
     using C = RowCfg<N>;
-    constexpr int TPL = tpl_of(N);
+    constexpr int TPL = row_tpl_of(N);
     constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;
     constexpr int NT = C::GROUPS * TPL * GR;
     constexpr int ROWS = C::GROUPS * GR;
     constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
-                            (FIRST ? 0 : (size_t)ROWS * N * sizeof(float4));
+                            (FIRST || !row_staged(N) ? 0 : (size_t)ROWS * N * sizeof(float4));
     auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN>;
     static int cap = 0;
     if (set_attr) {

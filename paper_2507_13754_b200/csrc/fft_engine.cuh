@@ -210,6 +210,10 @@ __host__ __device__ constexpr int conv_smem_bytes(int N, int T) {
     return conv_stage_offset(N, T) + N * T * 8 + (conv_p2_in_smem(N, T) ? conv_lutc_entries(N) * 8 + N * 8 : 0);
 }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
+// k_row: threads per row, and whether the W row is staged by a bulk copy a tile ahead.  N = 4096 runs two
+// items per thread and reads W directly: with the 64 KB staging buffer only one row would fit an SM.
+__host__ __device__ constexpr int row_tpl_of(int N) { return N == 4096 ? 128 : tpl_of(N); }
+__host__ __device__ constexpr bool row_staged(int N) { return N < 4096; }
 template <int GT>
 __device__ __forceinline__ void group_sync(int gid) {
     if (GT <= 32) __syncwarp();

@@ -206,20 +206,22 @@ struct RowArgs {
 // GROUPS; the W rows of its next tile arrive by one bulk copy (completion on the group's mbarrier)
 // in a staging buffer while the current tile computes.
 template <int N, int GROUPS, int MINB, bool FIRST, bool GEN>
-__global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), MINB) k_row(RowArgs a) {
+__global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) : 32), MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
     constexpr int NBL = N / RL;
     constexpr int M = 2 * N;
-    constexpr int TPL = tpl_of(N);
+    constexpr int TPL = row_tpl_of(N);
+    constexpr bool STAGED = row_staged(N);
     constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;  // rows per group
     constexpr int GT = TPL * GR;                   // threads per group
     constexpr int NT = GROUPS * GT;
     constexpr int ROWS = GROUPS * GR;
     constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(S1 % TPL == 0, "items per thread");
+    constexpr bool EARLY = NITEM * R1 <= 16;  // p and V requested a barrier ahead (else per item: registers)
     using Lay = LineLay<N>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [ROWS][PITCH] work area, both halves per slot
@@ -245,7 +247,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
         if (tid == 0)
             for (int i = 0; i < GROUPS; ++i) mbar_init(&mbar[i], 1);
         __syncthreads();
-        if (gl == 0 && gt < ngt) {
+        if (STAGED && gl == 0 && gt < ngt) {
             mbar_expect_tx(&mbar[g], TILE_BYTES);
             bulk_g2s(stg + g * GR * N, a.W + (long long)gt * GR * M, TILE_BYTES, &mbar[g]);
         }
@@ -257,7 +259,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
     while (gt < ngt) {
         const int row = gt * GR + gl / TPL;
         float wrow = a.scale;
-        float2 pold[NITEM][R1], vpot[NITEM][R1];
+        float2 pold[EARLY ? NITEM : 1][R1], vpot[EARLY ? NITEM : 1][R1];
         if (!FIRST) {
             // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
             // pull the p and V rows of this tile towards L2 while the W rows arrive
@@ -268,15 +270,18 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             }
             wrow *= __ldg(&a.ay[row % a.ny]);
             if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
-            mbar_wait(&mbar[g], phase);
-            phase ^= 1u;
+            if (STAGED) {
+                mbar_wait(&mbar[g], phase);
+                phase ^= 1u;
+            }
+            const float4 *wrow_g = reinterpret_cast<const float4 *>(a.W + (long long)row * M);
             // first inverse stage (contiguous blocks of RL) from the staged rows
 #pragma unroll 1
             for (int b = lt; b < NBL; b += TPL) {
                 P2 v[RL];
 #pragma unroll
                 for (int k = 0; k < RL; ++k) {
-                    const float4 f = stg[l * N + k * NBL + b];
+                    const float4 f = STAGED ? stg[l * N + k * NBL + b] : wrow_g[k * NBL + b];
                     v[k] = P2{make_float2(f.x, f.z), make_float2(f.y, f.w)};
                 }
                 pbfly<RL, +1>(v);
@@ -288,7 +293,7 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             if (gl == 0) {
                 const int nxt = gstride + (int)atomicAdd(&a.ctl->next_tile, 1u);
                 next_gt[g] = nxt;
-                if (nxt < ngt) {
+                if (STAGED && nxt < ngt) {
                     mbar_expect_tx(&mbar[g], TILE_BYTES);
                     bulk_g2s(stg + g * GR * N, a.W + (long long)nxt * GR * M, TILE_BYTES, &mbar[g]);
                 }
@@ -296,14 +301,16 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             if (R2 > 0) pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
             // request the running field and the potential at the thread's output points now: their
             // latency passes under the barrier and the shared-memory loads of the last inverse stage
+            if (EARLY) {
 #pragma unroll
-            for (int it = 0; it < NITEM; ++it)
+                for (int it = 0; it < NITEM; ++it)
 #pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    const long long gi = (long long)row * N + lt + it * TPL + j * S1;
-                    pold[it][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
-                    vpot[it][j] = __ldg(&a.V[gi]);
-                }
+                    for (int j = 0; j < R1; ++j) {
+                        const long long gi = (long long)row * N + lt + it * TPL + j * S1;
+                        pold[it][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
+                        vpot[it][j] = __ldg(&a.V[gi]);
+                    }
+            }
             if (R2 > 0) group_sync<GT>(g);
         }
         // last inverse stage + crop + window + accumulate + V.u + first forward stage; a thread
@@ -315,32 +322,63 @@ __global__ void __launch_bounds__(GROUPS * (tpl_of(N) >= 32 ? tpl_of(N) : 32), M
             float2 x[R1];
             float2 wre[R1], wim[R1];
             load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
+            constexpr int pi = EARLY ? 1 : 0;
+            const int ii = it * pi;  // slot of this item's p and V values
             if (!FIRST) {
+                if (!EARLY) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) {
+                        const long long gi = (long long)row * N + t + j * S1;
+                        pold[0][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
+                        vpot[0][j] = __ldg(&a.V[gi]);
+                    }
+                }
                 plast_inv_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
+                // The run-time options of the general variant are tested around whole loops over the R1
+                // outputs, never inside them: the loop bodies stay branch-free and interleave.
+                float2 uv[R1];
 #pragma unroll
                 for (int j = 0; j < R1; ++j) {
-                    const int pos = t + j * S1;
-                    const long long gi = (long long)row * N + pos;
-                    const float wgt = wrow * __ldg(&a.ax[pos]);
-                    float2 u = make_float2(x[j].x * wgt, x[j].y * wgt);
-                    if (GEN && a.ucbs) {
-                        // convergent Born series: u_{n+1} = u_n + gamma (A G(V u_n) - u_n), gamma = i V / eps
-                        const float2 gam = make_float2(-vpot[it][j].y * a.inv_e, vpot[it][j].x * a.inv_e);
-                        const float2 uo = term > 0 ? a.ucbs[gi] : make_float2(0.f, 0.f);
-                        u = cadd(uo, cmul(gam, csub(u, uo)));
-                        a.ucbs[gi] = u;
-                    }
-                    const float2 pv = cadd(pold[it][j], u);
-                    a.p[gi] = pv;
-                    if (!GEN || a.crit_row < 0) {
-                        uu = fmaf(u.x, u.x, fmaf(u.y, u.y, uu));
-                        pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
-                    } else if (row == a.crit_row) {  // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row
-                        uu += hypotf(u.x, u.y);  // hypotf: no underflow of the squares for very small fields
-                        pp += hypotf(pold[it][j].x, pold[it][j].y);
-                    }
-                    x[j] = cmul(vpot[it][j], u);
+                    const float wgt = wrow * __ldg(&a.ax[t + j * S1]);
+                    uv[j] = make_float2(x[j].x * wgt, x[j].y * wgt);
                 }
+                if (GEN && a.ucbs) {
+                    // convergent Born series: u_{n+1} = u_n + gamma (A G(V u_n) - u_n), gamma = i V / eps
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) {
+                        const long long gi = (long long)row * N + t + j * S1;
+                        const float2 gam = make_float2(-vpot[ii][j].y * a.inv_e, vpot[ii][j].x * a.inv_e);
+                        const float2 uo = term > 0 ? a.ucbs[gi] : make_float2(0.f, 0.f);
+                        uv[j] = cadd(uo, cmul(gam, csub(uv[j], uo)));
+                        a.ucbs[gi] = uv[j];
+                    }
+                }
+                if (!GEN || a.crit_row < 0) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) {
+                        const float2 pv = cadd(pold[ii][j], uv[j]);
+                        a.p[(long long)row * N + t + j * S1] = pv;
+                        uu = fmaf(uv[j].x, uv[j].x, fmaf(uv[j].y, uv[j].y, uu));
+                        pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
+                    }
+                } else if (row != a.crit_row) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) a.p[(long long)row * N + t + j * S1] = cadd(pold[ii][j], uv[j]);
+                } else {
+                    // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row; moduli through a 2^20 pre-scale
+                    // (the squares stay in range for 1e-25 < |.| < 1e13)
+                    constexpr float SC = 1048576.f, ISC = 1.f / 1048576.f;
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) {
+                        const float2 po = pold[ii][j];
+                        a.p[(long long)row * N + t + j * S1] = cadd(po, uv[j]);
+                        const float ax = uv[j].x * SC, ay = uv[j].y * SC, bx = po.x * SC, by = po.y * SC;
+                        uu = fmaf(sqrtf(fmaf(ax, ax, ay * ay)), ISC, uu);
+                        pp = fmaf(sqrtf(fmaf(bx, bx, by * by)), ISC, pp);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < R1; ++j) x[j] = cmul(vpot[ii][j], uv[j]);
                 if (!a.do_fwd) continue;
             } else {
 #pragma unroll
