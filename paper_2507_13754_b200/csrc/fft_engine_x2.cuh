@@ -58,21 +58,91 @@ __device__ __forceinline__ P2 pmul_w16(P2 d, int idx16) {
     }
 }
 
-// DFT_R of v (sign SGN), natural order in, BIT-REVERSED order out, both halves at once.
-template <int R, int SGN>
-__device__ __forceinline__ void pbfly(P2 (&v)[R]) {
+// w_16^idx = (w16x, SGN * w16y), idx = 0..7.
+__device__ __forceinline__ constexpr float w16x(int idx) {
+    constexpr float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f, H = 0.70710678118654752f;
+    return idx == 0 ? 1.f : idx == 1 ? C1 : idx == 2 ? H : idx == 3 ? S1 : idx == 4 ? 0.f : idx == 5 ? -S1 : idx == 6 ? -H : -C1;
+}
+__device__ __forceinline__ constexpr float w16y(int idx) {
+    constexpr float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f, H = 0.70710678118654752f;
+    return idx == 0 ? 0.f : idx == 1 ? S1 : idx == 2 ? H : idx == 3 ? C1 : idx == 4 ? 1.f : idx == 5 ? C1 : idx == 6 ? H : S1;
+}
+
+// Butterfly with the twiddle of its second operand folded in: s = a + b w, d = a - b w = 2a - s.
+// b w is never formed: 6 packed operations instead of 4 (multiply) + 4 (add, subtract).
+__device__ __forceinline__ void pbfly_tw(P2 a, P2 b, float2 wre, float2 wim, P2 &s, P2 &d) {
+    s.re = __ffma2_rn(b.re, wre, __ffma2_rn(b.im, neg2(wim), a.re));
+    s.im = __ffma2_rn(b.re, wim, __ffma2_rn(b.im, wre, a.im));
+    d.re = __ffma2_rn(a.re, f2(2.0f), neg2(s.re));
+    d.im = __ffma2_rn(a.im, f2(2.0f), neg2(s.im));
+}
+
+// Radix-2 layers h = H0 .. 1 of the DFT_R butterfly.  pend[i] is the power of w_16 that v[i] still has
+// to be multiplied by (all indices are compile-time constants after unrolling): a factor owed by the
+// first operand of a butterfly is applied there, one owed by the second operand goes into pbfly_tw.
+template <int R, int SGN, int H0>
+__device__ __forceinline__ void pbfly_layers(P2 (&v)[R], int (&pend)[R]) {
 #pragma unroll
-    for (int h = R / 2; h >= 1; h >>= 1) {
+    for (int h = H0; h >= 1; h >>= 1) {
 #pragma unroll
         for (int g = 0; g < R; g += 2 * h) {
 #pragma unroll
             for (int m = 0; m < h; ++m) {
-                const P2 a = v[g + m], b = v[g + m + h];
-                v[g + m] = padd(a, b);
-                v[g + m + h] = pmul_w16<SGN>(psub(a, b), m * (8 / h));
+                const int ia = g + m, ib = g + m + h;
+                const P2 a = pmul_w16<SGN>(v[ia], pend[ia]);
+                const int pb = pend[ib];
+                if (pb == 0 || pb == 4) {
+                    const P2 b = pmul_w16<SGN>(v[ib], pb);
+                    v[ia] = padd(a, b);
+                    v[ib] = psub(a, b);
+                } else {
+                    pbfly_tw(a, v[ib], f2(w16x(pb)), f2((float)SGN * w16y(pb)), v[ia], v[ib]);
+                }
+                pend[ia] = 0;
+                pend[ib] = m * (8 / h);
             }
         }
     }
+}
+
+// DFT_R of v (sign SGN), natural order in, BIT-REVERSED order out, both halves at once.
+template <int R, int SGN>
+__device__ __forceinline__ void pbfly(P2 (&v)[R]) {
+    int pend[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) pend[i] = 0;
+    pbfly_layers<R, SGN, R / 2>(v, pend);
+}
+
+// Inverse (DIT) butterfly with its input twiddles: DFT_R(+1) of v[k] conj(w[k]), w[k] = (wre[k], wim[k])
+// per half (w[0] too: the odd half carries the padding twist).  The twiddles of the upper half go into
+// the first layer.
+template <int R>
+__device__ __forceinline__ void pbfly_dit(P2 (&v)[R], const float2 (&wre)[R], const float2 (&wim)[R]) {
+    constexpr int h = R / 2;
+    int pend[R];
+#pragma unroll
+    for (int m = 0; m < h; ++m) {
+        const P2 a = pmulc2(v[m], wre[m], wim[m]);
+        pbfly_tw(a, v[m + h], wre[m + h], neg2(wim[m + h]), v[m], v[m + h]);
+        pend[m] = 0;
+        pend[m + h] = m * (8 / h);
+    }
+    pbfly_layers<R, +1, R / 4>(v, pend);
+}
+// the same with one scalar twiddle per position (both halves); w[0] = 1 is not applied
+template <int R>
+__device__ __forceinline__ void pbfly_dit(P2 (&v)[R], const float2 (&tw)[R]) {
+    constexpr int h = R / 2;
+    int pend[R];
+#pragma unroll
+    for (int m = 0; m < h; ++m) {
+        const P2 a = m > 0 ? pmulc(v[m], tw[m]) : v[0];
+        pbfly_tw(a, v[m + h], f2(tw[m + h].x), f2(-tw[m + h].y), v[m], v[m + h]);
+        pend[m] = 0;
+        pend[m + h] = m * (8 / h);
+    }
+    pbfly_layers<R, +1, R / 4>(v, pend);
 }
 
 __device__ __forceinline__ P2 lds_p2(const float4 *p) {
@@ -102,21 +172,19 @@ __device__ __forceinline__ void pstage_item_tw(float4 *sm, const float2 (&tw)[R]
     if (FWD) {
 #pragma unroll
         for (int j = 0; j < R; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j * S));
-                pbfly<R, -1>(v);
+        pbfly<R, -1>(v);
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const int k = brev(i, R);
             if (S > 1 && k > 0) v[i] = pmul(v[i], tw[k]);
         }
-    #pragma unroll
+#pragma unroll
         for (int i = 0; i < R; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, R) * S), v[i]);
     } else {
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = lds_p2(sm + Lay::addr(line, base + k * S));
-    #pragma unroll
-        for (int k = 0; k < R; ++k)
-            if (S > 1 && k > 0) v[k] = pmulc(v[k], tw[k]);
-        pbfly<R, +1>(v);
+        if (S > 1) pbfly_dit<R>(v, tw);
+        else pbfly<R, +1>(v);
 #pragma unroll
         for (int i = 0; i < R; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, R) * S), v[i]);
     }
@@ -183,9 +251,7 @@ __device__ __forceinline__ void plast_inv_tw(float2 (&z)[R1], int line, int t, c
     P2 v[R1];
 #pragma unroll
     for (int k = 0; k < R1; ++k) v[k] = lds_p2(sm + Lay::addr(line, t + k * S1));
-#pragma unroll
-    for (int k = 0; k < R1; ++k) v[k] = pmulc2(v[k], wre[k], wim[k]);
-    pbfly<R1, +1>(v);
+    pbfly_dit<R1>(v, wre, wim);
 #pragma unroll
     for (int i = 0; i < R1; ++i) {
         const int j = brev(i, R1);
@@ -234,28 +300,59 @@ __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, cons
     for (int j = 0; j < RL; ++j) v[j] = lds_p2(sm + Lay::addr(line, base + j));
     pbfly<RL, -1>(v);
     P2 u[RL];
+    if (!KABS) {
+        // u[k] = X[k] (alpha + i) r, r = 1/(alpha^2 + 1), goes straight into the inverse butterfly: the r of a
+        // second operand is folded into the first layer (s = a + t r, d = a - t r), so t r is never formed.
+        constexpr int h = RL / 2;
+        float2 rr[h];
 #pragma unroll
-    for (int i = 0; i < RL; ++i) {
-        const int k = brev(i, RL);
-        const float2 al = __fadd2_rn(pp[k], f2(a_line));
-        const float2 d = __ffma2_rn(al, al, f2(1.0f));
-        const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
-        P2 w = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};
-        if (KABS && ka.nu > 0.f) {
-            // kappa^nu = exp2(nu/2 log2(kappa^2)); frequencies masked for the periodic boundary (alpha ~ 1e18) give 0
-            float2 q = __ffma2_rn(al, f2(ka.e), f2(1.0f));  // kappa^2 = |p|^2/k0^2 (>= 0 up to rounding)
-            q = make_float2(fmaxf(q.x, 0.f), fmaxf(q.y, 0.f));
-            const float2 lg = make_float2(__log2f(q.x), __log2f(q.y));
-            const float2 kn = make_float2(exp2f(0.5f * ka.nu * lg.x), exp2f(0.5f * ka.nu * lg.y));
-            const float2 k1 = make_float2(exp2f(0.5f * lg.x), exp2f(0.5f * lg.y));
-            const float2 ok = make_float2(al.x < 1.0e17f ? 1.f : 0.f, al.y < 1.0e17f ? 1.f : 0.f);
-            const float2 vr = __fmul2_rn(__fmul2_rn(__fmul2_rn(kn, k1), f2(ka.B)), ok);                    // Re VV/k0^2
-            const float2 vi = __fmul2_rn(neg2(__ffma2_rn(kn, f2(ka.A), f2(ka.e))), ok);                    // Im VV/k0^2
-            w = P2{__ffma2_rn(w.re, vr, neg2(__fmul2_rn(w.im, vi))), __ffma2_rn(w.re, vi, __fmul2_rn(w.im, vr))};
+        for (int i = 0; i < RL; ++i) {
+            const int k = brev(i, RL);
+            const float2 al = __fadd2_rn(pp[k], f2(a_line));
+            const float2 d = __ffma2_rn(al, al, f2(1.0f));
+            const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
+            const P2 t = P2{__ffma2_rn(v[i].re, al, neg2(v[i].im)), __ffma2_rn(v[i].im, al, v[i].re)};
+            if (k < h) {
+                u[k] = P2{__fmul2_rn(t.re, r), __fmul2_rn(t.im, r)};
+            } else {
+                u[k] = t;
+                rr[k - h] = r;
+            }
         }
-        u[k] = w;
+        int pend[RL];
+#pragma unroll
+        for (int m = 0; m < h; ++m) {
+            const P2 a = u[m], t = u[m + h];
+            u[m] = P2{__ffma2_rn(t.re, rr[m], a.re), __ffma2_rn(t.im, rr[m], a.im)};
+            u[m + h] = P2{__ffma2_rn(t.re, neg2(rr[m]), a.re), __ffma2_rn(t.im, neg2(rr[m]), a.im)};
+            pend[m] = 0;
+            pend[m + h] = m * (8 / h);
+        }
+        pbfly_layers<RL, +1, RL / 4>(u, pend);
+    } else {
+#pragma unroll
+        for (int i = 0; i < RL; ++i) {
+            const int k = brev(i, RL);
+            const float2 al = __fadd2_rn(pp[k], f2(a_line));
+            const float2 d = __ffma2_rn(al, al, f2(1.0f));
+            const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
+            P2 w = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};
+            if (KABS && ka.nu > 0.f) {
+                // kappa^nu = exp2(nu/2 log2(kappa^2)); frequencies masked for the periodic boundary (alpha ~ 1e18) give 0
+                float2 q = __ffma2_rn(al, f2(ka.e), f2(1.0f));  // kappa^2 = |p|^2/k0^2 (>= 0 up to rounding)
+                q = make_float2(fmaxf(q.x, 0.f), fmaxf(q.y, 0.f));
+                const float2 lg = make_float2(__log2f(q.x), __log2f(q.y));
+                const float2 kn = make_float2(exp2f(0.5f * ka.nu * lg.x), exp2f(0.5f * ka.nu * lg.y));
+                const float2 k1 = make_float2(exp2f(0.5f * lg.x), exp2f(0.5f * lg.y));
+                const float2 ok = make_float2(al.x < 1.0e17f ? 1.f : 0.f, al.y < 1.0e17f ? 1.f : 0.f);
+                const float2 vr = __fmul2_rn(__fmul2_rn(__fmul2_rn(kn, k1), f2(ka.B)), ok);                    // Re VV/k0^2
+                const float2 vi = __fmul2_rn(neg2(__ffma2_rn(kn, f2(ka.A), f2(ka.e))), ok);                    // Im VV/k0^2
+                w = P2{__ffma2_rn(w.re, vr, neg2(__fmul2_rn(w.im, vi))), __ffma2_rn(w.re, vi, __fmul2_rn(w.im, vr))};
+            }
+            u[k] = w;
+        }
+        pbfly<RL, +1>(u);
     }
-    pbfly<RL, +1>(u);
 #pragma unroll
     for (int i = 0; i < RL; ++i) sts_p2(sm + Lay::addr(line, base + brev(i, RL)), u[i]);
 }
