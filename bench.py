@@ -37,11 +37,11 @@ ALG_BYTES = {2: {"k_row": 56.0, "k_conv": 32.0},
 #   traffic  = dram__bytes_read.sum + dram__bytes_write.sum
 #   fp32_res = FP32 results issued (packed instructions count twice), from smsp__inst_executed x mix
 NCU = {
-    "cfg3": {"k_conv": {"traffic": 67.22e6 + 17.68e6, "fp32_res": 35.74e6 * 32 * (2 * 0.545 + 0.058)},
-             "k_row": {"traffic": 134.32e6 + 47.00e6, "fp32_res": 19.34e6 * 32 * (2 * 0.471 + 0.141)}},
-    "cfg5": {"k_conv_z": {"traffic": 536.93e6 + 484.54e6, "fp32_res": 193.32e6 * 32 * (2 * 0.580 + 0.098)},
-             "k_col_fwd_y": {"traffic": 268.47e6 + 479.94e6, "fp32_res": 80.53e6 * 32 * 0.672},
-             "k_row": {"traffic": 536.96e6 + 346.34e6, "fp32_res": 62.35e6 * 32 * (2 * 0.408 + 0.185)}},
+    "cfg3": {"k_conv": {"traffic": 67.21e6 + 16.79e6, "fp32_res": 34.96e6 * 32 * (2 * 0.535 + 0.058)},
+             "k_row": {"traffic": 134.32e6 + 44.00e6, "fp32_res": 19.08e6 * 32 * (2 * 0.456 + 0.143)}},
+    "cfg5": {"k_conv_z": {"traffic": 536.93e6 + 484.53e6, "fp32_res": 190.56e6 * 32 * (2 * 0.568 + 0.099)},
+             "k_col_fwd_y": {"traffic": 268.47e6 + 481.34e6, "fp32_res": 83.53e6 * 32 * 0.648},
+             "k_row": {"traffic": 536.98e6 + 345.34e6, "fp32_res": 61.11e6 * 32 * (2 * 0.398 + 0.189)}},
 }
 FP32_PEAK = 148 * 128 * 1.965e9   # FP32 results/s: 128 lanes/clk/SM (packed f32x2 counts as 2 results, same pipe)
 
