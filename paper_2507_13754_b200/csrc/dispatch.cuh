@@ -116,7 +116,7 @@ static cudaError_t launch_conv_t(const ColArgs &a, const CUtensorMap *tmap, int 
         cudaError_t e = launch_conv_tt<N, false>(a, tmap, n_outer, st, true);
         return e != cudaSuccess ? e : launch_conv_tt<N, true>(a, tmap, n_outer, st, true);
     }
-    return a.kabs.nu > 0.f ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false)
+    return a.kabs.nu > 0.f || a.masked ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false)
                            : launch_conv_tt<N, false>(a, tmap, n_outer, st, false);
 }
 

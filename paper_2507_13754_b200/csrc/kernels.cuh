@@ -46,6 +46,7 @@ struct ColArgs {
     const float *p2_outer;  // [n_outer] of the outer axis or nullptr             (CONV)
     float inv_e;            // k0^2/eps = 1/damping
     KAbs kabs;              // k-space multiplier potential of Eq. 24 (k_conv<..., KABS = true> only)
+    int masked;             // periodic boundary: axis tables mask the odd padded frequencies (general k_conv)
     Luts lut;
     const Ctl *ctl;
 };
@@ -551,9 +552,19 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         const int inner0 = (tile % tiles) * T;
         const int outer = tile / tiles;
         const bool more = tile + (int)gridDim.x < total;
+        // alpha of a line from the other axes.  General variant (KABS): a line at a frequency the periodic
+        // boundary masks (axis tables hold 1e18 there) gives exact zeros and is not computed.
+        auto line_alpha = [&](int in0, int out) {
+            float al = __ldg(&a.p2_inner[in0 + line]) - 1.0f;
+            if (a.p2_outer) al += __ldg(&a.p2_outer[out]);
+            return al * a.inv_e;
+        };
+        float a_line = 0.f;
+        if (KABS) a_line = line_alpha(inner0, outer);
+        const bool dead = KABS && a_line > 1.0e17f;
         if (R2 > 0) {
-            pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
-            group_sync<GT>(g);
+            if (!dead) pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
+            group_sync<GT>(g);  // by every line: lines of different state may share a warp
             // by now the store of the previous tile has been read out of the buffer: refill it
             if (tid == 0 && to_load >= 0 && tile != (int)blockIdx.x) {
                 bulk_wait_read();
@@ -561,18 +572,16 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             }
             if (tile != (int)blockIdx.x) to_load = to_load >= 0 && to_load + (int)gridDim.x < total ? to_load + (int)gridDim.x : -1;
         }
-        {
-            float a_line = __ldg(&a.p2_inner[inner0 + line]) - 1.0f;
-            if (a.p2_outer) a_line += __ldg(&a.p2_outer[outer]);
-            a_line *= a.inv_e;
+        if (!dead) {
+            if (!KABS) a_line = line_alpha(inner0, outer);
             KAbs ka = a.kabs;
             if (KABS && a.ctl->term == 0) ka.nu = 0.f;  // term 0 is u_0 = A G S: the plain Green's spectrum
 #pragma unroll 1
             for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line, ka);
-            group_sync<GT>(g);
         }
+        group_sync<GT>(g);
         if (R2 > 0) {
-            pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
+            if (!dead) pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             group_sync<GT>(g);
         }
         // ---- fused: last inverse stage of this tile, first forward stage of the next one ----
@@ -580,19 +589,29 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             mbar_wait(&mbar, phase);
             phase ^= 1u;
         }
+        bool dead_next = false;  // the same line of the next tile (another outer index in 3-D)
+        if (KABS && more) {
+            const int nt = tile + (int)gridDim.x;
+            dead_next = line_alpha((nt % tiles) * T, nt / tiles) > 1.0e17f;
+        }
 #pragma unroll 1
         for (int t = lt; t < S1; t += TPL) {
             float2 wre[R1], wim[R1];
             load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
             float2 z[R1], x[R1];
-            plast_inv_tw<N, R1, Lay>(z, line, t, wk, wre, wim);
+            if (!dead) {
+                plast_inv_tw<N, R1, Lay>(z, line, t, wk, wre, wim);
+            } else {
+#pragma unroll
+                for (int j = 0; j < R1; ++j) z[j] = make_float2(0.f, 0.f);
+            }
 #pragma unroll
             for (int j = 0; j < R1; ++j) {
                 float2 &e = io_at(t + j * S1);
                 x[j] = e;
                 e = z[j];
             }
-            if (more) pfirst_fwd_tw<N, R1, Lay>(x, line, t, wk, wre, wim);
+            if (more && !dead_next) pfirst_fwd_tw<N, R1, Lay>(x, line, t, wk, wre, wim);
         }
         fence_async_smem();
         __syncthreads();  // result tile complete, next input consumed, next first stage in place

@@ -129,6 +129,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     a.ctl = f.ctl;
     a.inv_e = (float)(1.0 / pl->damping);
     a.kabs = f.kabs;
+    a.masked = pl->boundary == TBS_BOUNDARY_PERIODIC;
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
