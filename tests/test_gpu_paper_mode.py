@@ -53,6 +53,47 @@ def test_periodic_boundary_matches_oracle_pad_factor_one():
     compare_fields(res.p[0].cpu().numpy(), ref.p, "periodic 128^2")
 
 
+def test_periodic_boundary_512_matches_oracle_pad_factor_one():
+    """N = 512: a line is owned by a whole warp, so k_conv skips the masked (odd-frequency) columns outright."""
+    N, abl = 512, 32
+    case = _case(N, abl)
+    V, S, g, win = _oracle_inputs(N, abl, *case)
+    ref = R.solve(V, S, g, 40, 0.0, pad=1, windows=win)
+    res = _plan(N, abl, *case).solve(40, 0.0)
+    assert int(res.n_terms[0]) == ref.n_terms == 40
+    compare_fields(res.p[0].cpu().numpy(), ref.p, "periodic 512^2, 40 terms")
+    compare_history(res.history[0], ref.history, 40)
+
+
+def test_periodic_boundary_3d_matches_oracle_pad_factor_one():
+    """3-D: in the z pass whole tiles sit at a masked ky and the state of a line changes from tile to tile."""
+    from paper_2507_13754_b200.tbs import Plan
+    N, abl = 32, 6
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / 6.0
+    rng = np.random.default_rng(3 * N)
+    c = (c0 * (1 + 0.02 * rng.standard_normal((N, N, N)))).astype(np.float32)
+    ii = np.arange(N // 2 - 4, N // 2 + 5)
+    gy, gx = np.meshgrid(ii, ii, indexing="ij")
+    pos = np.stack([gx.ravel() * dx, gy.ravel() * dx, np.full(gx.size, (abl + 3) * dx)], 1)
+    amp = np.full((1, pos.shape[0]), 1.0 - 0.5j, dtype=np.complex64)
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    V = R.potential(c.astype(np.float64), 0.5, 1.1, f, c0, 0.8)
+    S = R.deposit((N, N, N), dx, pos, amp[0])
+    g = R.green_spectrum((N, N, N), dx, k0, eps)
+    win = tuple(R.abl_window(N, abl) for _ in range(3))
+    ref = R.solve(V, S, g, 2000, 1e-6, pad=1, windows=win)
+    plan = Plan((N, N, N), dx, [f], c0, 0.8)
+    plan.set_boundary("periodic")
+    plan.set_abl(abl, 9.666)
+    plan.set_medium(torch.from_numpy(c).cuda(), alpha0_db=0.5, y=1.1)
+    plan.set_source(pos, amp)
+    res = plan.solve(2000, 1e-6)
+    assert res.status == 0 and ref.status == R.OK
+    assert abs(int(res.n_terms[0]) - ref.n_terms) <= 1
+    compare_fields(res.p[0].cpu().numpy(), ref.p, "periodic 32^3")
+
+
 def test_paper_mode_matches_oracle_algorithm_1():
     N, abl = 256, 32
     case = _case(N, abl)
