@@ -11,7 +11,9 @@
  * Conventions
  *  - Every array is row-major with x fastest: index = (z*Ny + y)*Nx + x.
  *  - complex64 = interleaved float (re, im).  "dev" = CUDA device pointer, "host" = host pointer.
- *  - The caller owns every buffer it passes in.  The plan owns V, S, p and the FFT workspaces.
+ *  - The caller owns every buffer it passes in.  V, S, p of every frequency and the FFT intermediates live in
+ *    one device range, the workspace: the caller's (tbs_plan_set_workspace, e.g. a torch allocation) or, when
+ *    none was given by the first call that needs it, the plan's own.
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *  - No exception crosses the ABI: every call returns a tbs_status; tbs_last_error() gives text.
  *  - A plan is not thread-safe; distinct plans are independent.
@@ -39,7 +41,7 @@ typedef enum {
     TBS_ERR_UNSUPPORTED_SIZE = -2,
     TBS_ERR_NOT_READY = -3,      /* medium or source not set */
     TBS_ERR_CUDA = -4,
-    TBS_ERR_DIVERGED = -5,       /* a term norm became non-finite (||GV|| >= 1) */
+    TBS_ERR_DIVERGED = -5,       /* the series diverges (||GV|| >= 1): see tbs_solve */
     TBS_ERR_ALLOC = -6
 } tbs_status;
 
@@ -57,8 +59,27 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
                            const double *f_hz, double c0, double damping);
 void tbs_plan_destroy(tbs_plan *plan);
 
-/* Device bytes the plan holds (fields + workspaces). */
+/* Workspace (inputs of Alg. 1, held on the device).  tbs_plan_workspace_bytes: the size the
+ * plan needs -- V, S and p [n] complex64 per frequency, the x-transformed rows W1 [nz ny][2 nx] and, in 3-D, the
+ * y/z-transformed W2 [nz][2 ny][2 nx], the latter two once per series in flight (one, or two for nfreq > 1),
+ * every region rounded up to 256 bytes -- known as soon as the plan exists.  tbs_plan_set_workspace: run in
+ * caller-owned device memory (dev_ptr 256-byte aligned, bytes >= the size above; it must outlive the plan or the
+ * next call of this function).  Contents are undefined afterwards: set medium and source (again).  Without this
+ * call the plan allocates the same range itself at the first call that needs it.
+ * tbs_plan_device_bytes: device bytes the plan itself has allocated (tables, control, and its own workspace). */
 size_t tbs_plan_workspace_bytes(const tbs_plan *plan);
+tbs_status tbs_plan_set_workspace(tbs_plan *plan, void *dev_ptr, size_t bytes);
+size_t tbs_plan_device_bytes(const tbs_plan *plan);
+
+/* The m-th frequency a periodic n-point grid of spacing dx_m carries exactly, m c0/(n dx) -- the paper picks its
+ * frequency this way (f = 55 v_f/(4096 dx) = 1 007 080 Hz).  0 for non-positive arguments. */
+double tbs_grid_harmonic_frequency(int m, double c0, int n, double dx_m);
+
+/* Frequency batch (nfreq > 1): how many members are solved at once, 1 or 2 (default 2).  With 2, two series run
+ * on streams of the plan's own with grids sized for half of the SMs each, so that the HBM-bound passes of one
+ * overlap the FP32-bound convolution pass of the other; a member that has stopped hands its place to the next
+ * frequency.  The paper's harmonic loop is sequential. */
+tbs_status tbs_set_concurrency(tbs_plan *plan, int members);
 
 /* Text of the last error on this plan (plan-owned storage, valid until the next call). */
 const char *tbs_last_error(const tbs_plan *plan);
@@ -69,7 +90,8 @@ const char *tbs_last_error(const tbs_plan *plan);
  * dispersive = 0 drops the eta term (the "absorbing" row of Table 3).  The term update becomes
  * u_{n+1} = A F^-1[ghat(p) VV(|p|) F[u_n]]: the spatial potential is ignored (tbs_set_medium not needed)
  * and the multiplier is applied inside the fused Green's-spectrum stage.  alpha0_si = 0 switches back to the
- * spatial potential, which then has to be set again.  Not combined with TBS_SCHEME_CBS. */
+ * spatial potential, which then has to be set again; so does a later tbs_set_medium / tbs_set_potential (the two
+ * forms are not combined).  With TBS_SCHEME_CBS selected (or selecting it afterwards): TBS_ERR_INVALID_ARG. */
 tbs_status tbs_set_kspace_absorption(tbs_plan *plan, double alpha0_si, double nu, int dispersive);
 
 /* Boundary treatment (default TBS_BOUNDARY_PAD: zero-pad to 2N per axis, linear convolution, crop --
@@ -104,8 +126,9 @@ tbs_status tbs_set_abl(tbs_plan *plan, int cells, double zeta_half_mu);
 /* Medium -> potential, for every frequency of the plan (absorption from
  * Eq. 3 and Eq. 7):
  *   ktilde = w/c(r) + alpha (tan(pi y/2) + i), alpha = alpha0 w^y, V = ktilde^2 - k0^2 - i eps.
- *   c [n] dev float: sound speed map.  rho [n] dev float or NULL: density; it does not enter V
- *   (rho_s ~ rho_f); its mean (or rho0 when NULL) enters the harmonic source only.
+ *   c [n] dev float: sound speed map.  rho [n] dev float or NULL: density map; accepted and not read -- density
+ *   does not enter V (rho_s ~ rho_f).  rho0 > 0: the ambient density of xi = beta/(rho0 c0^4),
+ *   the constant of the harmonic sources; unused by a linear solve.
  *   alpha0_map [n] dev float or NULL (then the scalar alpha0_db_mhz_cm is used), dB/(MHz^y cm).
  *   y: power-law exponent, y != 1 unless alpha0 == 0.  beta = 1 + B/2A.
  * tbs_set_medium_host takes the same maps as HOST pointers and copies them itself. */
@@ -133,6 +156,9 @@ tbs_status tbs_set_source_field(tbs_plan *plan, int ifreq, const float *S, void 
  *   history [nfreq][max_terms+1] host doubles: history[k] = ||u_k||_2/||p_k||_2, history[0] = 1;
  *     entries after n_terms are 0.   n_terms [nfreq] host: index of the last term added.
  * Synchronises `stream` before returning.  Returns the worst status over frequencies.
+ * TBS_ERR_DIVERGED (field and history up to that term are still written): the measure became non-finite, or
+ * ||u_n|| exceeded 10^6 ||u_0||, or history[n] stayed above ten times its running minimum for 32 terms in a row
+ * (the paper only caps the iterations; convergence needs ||GV|| < 1).
  * Range: fields and norms are complex64 / fp32 partial sums; |u_n|^2 must stay inside the fp32 range, i.e.
  * term magnitudes between about 1e-19 and 1e19.  A series whose terms fall below that (harmonics 3-5 of a
  * source of arbitrary small strength) reports TBS_ERR_DIVERGED (0/0); scale the source, or use the
@@ -178,11 +204,11 @@ tbs_status tbs_green_spectrum(tbs_plan *plan, int ifreq, float *out, void *strea
  * loop measured with CUDA events on `stream`. */
 int64_t tbs_last_launch_count(const tbs_plan *plan);
 double tbs_last_loop_ms(const tbs_plan *plan);
-/* Per-kernel device time of ONE term (ms) for frequency ifreq: runs a live series (term 0, three
- * warm-up terms, then `reps` <= 256 terms, no graph) with a CUDA event recorded on `stream` between
- * consecutive kernels, and averages per kernel: out_ms[0] = row kernel K31, out_ms[1] = K2 (2-D) or
- * out_ms[1..3] = y-forward, z-convolution, y-inverse passes (3-D).  Requires medium and source;
- * overwrites the plan's running field. */
+/* Per-kernel device time of ONE term (ms) for frequency ifreq: after a live series of term 0 and three
+ * warm-up terms, each kernel of the term is launched `reps` <= 256 times back to back between two CUDA events
+ * on `stream` (no event between launches), and the average is returned: out_ms[0] = row kernel K31,
+ * out_ms[1] = K2 (2-D) or out_ms[1..3] = y-forward, z-convolution, y-inverse passes (3-D).  Requires medium
+ * and source; leaves the plan's running field and intermediates undefined. */
 tbs_status tbs_profile_term(tbs_plan *plan, int ifreq, int reps, double out_ms[4], void *stream);
 /* Terms per graph launch (default 16); 0 disables CUDA graphs (plain launches). */
 tbs_status tbs_set_graph_batch(tbs_plan *plan, int terms_per_graph);

@@ -210,10 +210,19 @@ __host__ __device__ constexpr int conv_smem_bytes(int N, int T) {
     return conv_stage_offset(N, T) + N * T * 8 + (conv_p2_in_smem(N, T) ? conv_lutc_entries(N) * 8 + N * 8 : 0);
 }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
+// k_conv: first/last-stage items per line >= threads of two lines (N = 512, 1024, 2048): the fused last/first
+// stage runs by line pairs with 16-byte accesses to the tile buffer.
+__host__ __device__ constexpr bool conv_pair_exchange(int N) { return N == 512 || N == 1024 || N == 2048; }
 // k_row: threads per row, and whether the W row is staged by a bulk copy a tile ahead.  N = 4096 runs two
 // items per thread and reads W directly: with the 64 KB staging buffer only one row would fit an SM.
 __host__ __device__ constexpr int row_tpl_of(int N) { return N == 4096 ? 128 : tpl_of(N); }
 __host__ __device__ constexpr bool row_staged(int N) { return N < 4096; }
+// Middle stage (radix R2, blocks of R2*RL, stride RL) and contiguous stage (blocks of RL) touch the same RL x RL
+// block from the same 16 threads when R2 == RL and both deal item b to thread b mod TPL: a warp barrier is
+// enough between them (the plans of N = 2048 and 4096).
+__host__ __device__ constexpr bool warp_local_mid(int R2, int RL, int TPL) {
+    return R2 > 0 && R2 == RL && RL == 16 && TPL >= 32 && TPL % 32 == 0;
+}
 template <int GT>
 __device__ __forceinline__ void group_sync(int gid) {
     if (GT <= 32) __syncwarp();

@@ -30,7 +30,16 @@ struct Ctl {
     unsigned int ticket;  // CTAs of the current k_row launch that have finished
     int n_terms;     // index of the last term added
     unsigned int next_tile;  // k_row: row tiles handed out beyond the first one of every group
+    // divergence guard (the paper only caps the iterations, and states that
+    // convergence needs ||GV|| < 1)
+    int hold;        // 1: never stop (tbs_profile_term times kernels on a series that may overflow)
+    int rising;      // consecutive terms with r_n above 10 x its running minimum
+    double rmin;     // running minimum of r_n, n >= 1
+    double uu0;      // ||u_0||^2
 };
+// r_n above 10 x its minimum for this many consecutive terms, or ||u_n|| above GROWTH_LIMIT ||u_0||: diverged
+constexpr int DIVERGE_RISING_TERMS = 32;
+constexpr double DIVERGE_GROWTH_SQ = 1.0e12;  // (1e6)^2 on the squared norms
 
 enum { MODE_FWD = 1, MODE_INV = 2 };
 
@@ -223,6 +232,9 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
     constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(S1 % TPL == 0, "items per thread");
     constexpr bool EARLY = NITEM * R1 <= 16;  // p and V requested a barrier ahead (else per item: registers)
+    // R2 == RL: the RL x RL block a middle-stage item works in is the block of the RL contiguous-stage items of the
+    // same 16 threads (item b of either stage lies in block b / RL), so the two stages only need a warp barrier.
+    constexpr bool WL = warp_local_mid(R2, RL, TPL);
     using Lay = LineLay<N>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [ROWS][PITCH] work area, both halves per slot
@@ -289,15 +301,23 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
                 for (int i = 0; i < RL; ++i) sts_p2(wk + Lay::addr(l, b * RL + brev(i, RL)), v[i]);
             }
-            group_sync<GT>(g);
-            // the group's staging rows are free: take the next tile and fetch its W rows
-            if (gl == 0) {
-                const int nxt = gstride + (int)atomicAdd(&a.ctl->next_tile, 1u);
-                next_gt[g] = nxt;
-                if (STAGED && nxt < ngt) {
-                    mbar_expect_tx(&mbar[g], TILE_BYTES);
-                    bulk_g2s(stg + g * GR * N, a.W + (long long)nxt * GR * M, TILE_BYTES, &mbar[g]);
+            // the group's staging rows are free once every thread of the group is past this point: take the next
+            // tile and fetch its W rows
+            auto fetch_next = [&]() {
+                if (gl == 0) {
+                    const int nxt = gstride + (int)atomicAdd(&a.ctl->next_tile, 1u);
+                    next_gt[g] = nxt;
+                    if (STAGED && nxt < ngt) {
+                        mbar_expect_tx(&mbar[g], TILE_BYTES);
+                        bulk_g2s(stg + g * GR * N, a.W + (long long)nxt * GR * M, TILE_BYTES, &mbar[g]);
+                    }
                 }
+            };
+            if (WL) {
+                __syncwarp();
+            } else {
+                group_sync<GT>(g);
+                fetch_next();
             }
             if (R2 > 0) pstage_line<N, S1, R2s, false, Lay, TPL>(wk, a.lut.C, l, lt);
             // request the running field and the potential at the thread's output points now: their
@@ -313,6 +333,7 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
                     }
             }
             if (R2 > 0) group_sync<GT>(g);
+            if (WL) fetch_next();
         }
         // last inverse stage + crop + window + accumulate + V.u + first forward stage; a thread
         // writes the slots it has just read, so the items need no barrier between them.  The p and V
@@ -399,7 +420,8 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
         // ---------------- forward half: the remaining stages of FFT_x ----------------
         if (R2 > 0) {
             pstage_line<N, S1, R2s, true, Lay, TPL>(wk, a.lut.C, l, lt);
-            group_sync<GT>(g);
+            if (WL) __syncwarp();
+            else group_sync<GT>(g);
         }
         // last forward stage (contiguous blocks of RL) straight to global memory.  A thread reads
         // exactly the slots it writes in the first inverse stage of its next tile.
@@ -445,7 +467,24 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
                 a.ctl->next_tile = 0;
                 a.ctl->n_terms = term;
                 a.ctl->term = term + 1;
-                if (!(r == r) || r > 1.0e300) {
+                // divergence guard: a non-finite measure; the term norm a million times that of u_0 (L2 measure);
+                // the measure above ten times its minimum for 32 terms in a row
+                bool diverged = !(r == r) || r > 1.0e300;
+                if (term == 0) {
+                    a.ctl->uu0 = nu;
+                    a.ctl->rmin = 1.0e300;
+                    a.ctl->rising = 0;
+                } else if (!diverged) {
+                    if ((!GEN || a.crit_row < 0) && nu > DIVERGE_GROWTH_SQ * a.ctl->uu0) diverged = true;
+                    const double rmin = a.ctl->rmin;
+                    if (r < rmin) a.ctl->rmin = r;
+                    const int rising = r > 10.0 * rmin ? a.ctl->rising + 1 : 0;
+                    a.ctl->rising = rising;
+                    if (rising >= DIVERGE_RISING_TERMS) diverged = true;
+                }
+                if (a.ctl->hold) {
+                    // profiling: keep going whatever the values
+                } else if (diverged) {
                     a.ctl->done = 1; a.ctl->status = -5;
                 } else if (term >= 1 && r < a.ctl->tol) {
                     a.ctl->done = 1; a.ctl->status = 0;
@@ -473,6 +512,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     constexpr int GT = TPL >= 32 ? TPL : 32;
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
+    constexpr bool WL = warp_local_mid(R2, RL, TPL);  // see k_row
+    // fused last/first stage by line pairs (see there): when the stage has an item for every thread of two lines
+    constexpr bool PAIRX = conv_pair_exchange(N) && (2 * TPL) % 32 == 0 && T / 2 <= 7;
     using Lay = LineLay<N>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
@@ -554,17 +596,19 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         const bool more = tile + (int)gridDim.x < total;
         // alpha of a line from the other axes.  General variant (KABS): a line at a frequency the periodic
         // boundary masks (axis tables hold 1e18 there) gives exact zeros and is not computed.
-        auto line_alpha = [&](int in0, int out) {
-            float al = __ldg(&a.p2_inner[in0 + line]) - 1.0f;
+        auto line_alpha_of = [&](int in0, int out, int ln) {
+            float al = __ldg(&a.p2_inner[in0 + ln]) - 1.0f;
             if (a.p2_outer) al += __ldg(&a.p2_outer[out]);
             return al * a.inv_e;
         };
+        auto line_alpha = [&](int in0, int out) { return line_alpha_of(in0, out, line); };
         float a_line = 0.f;
         if (KABS) a_line = line_alpha(inner0, outer);
         const bool dead = KABS && a_line > 1.0e17f;
         if (R2 > 0) {
             if (!dead) pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
-            group_sync<GT>(g);  // by every line: lines of different state may share a warp
+            if (WL) __syncwarp();
+            else group_sync<GT>(g);  // by every line: lines of different state may share a warp
             // by now the store of the previous tile has been read out of the buffer: refill it
             if (tid == 0 && to_load >= 0 && tile != (int)blockIdx.x) {
                 bulk_wait_read();
@@ -579,11 +623,14 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
 #pragma unroll 1
             for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line, ka);
         }
-        group_sync<GT>(g);
+        if (WL) __syncwarp();
+        else group_sync<GT>(g);
         if (R2 > 0) {
             if (!dead) pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
-            group_sync<GT>(g);
+            if (!PAIRX) group_sync<GT>(g);
         }
+        // pair exchange: the next stage reads both lines of the thread's pair
+        if (PAIRX) asm volatile("bar.sync %0, %1;" ::"r"(8 + tid / (2 * TPL)), "n"(2 * TPL) : "memory");
         // ---- fused: last inverse stage of this tile, first forward stage of the next one ----
         if (more) {
             mbar_wait(&mbar, phase);
@@ -594,24 +641,79 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             const int nt = tile + (int)gridDim.x;
             dead_next = line_alpha((nt % tiles) * T, nt / tiles) > 1.0e17f;
         }
+        if (PAIRX) {
+            // Pair exchange: a thread does this stage for BOTH lines of a 16-byte chunk of the tile buffer at its
+            // positions, so the buffer is read and written 16 bytes at a time (conflict-free under the TMA swizzle,
+            // half the instructions of the per-line 8-byte exchange) and the twiddles are fetched once per pair.
+            const int l0 = 2 * (tid / (2 * TPL)), pt = tid % (2 * TPL);
+            bool dp[2] = {false, false}, dn[2] = {false, false};
+            if (KABS) {
+                const int nt = tile + (int)gridDim.x;
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    dp[q] = line_alpha_of(inner0, outer, l0 + q) > 1.0e17f;
+                    dn[q] = more && line_alpha_of((nt % tiles) * T, nt / tiles, l0 + q) > 1.0e17f;
+                }
+            }
 #pragma unroll 1
-        for (int t = lt; t < S1; t += TPL) {
-            float2 wre[R1], wim[R1];
-            load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
-            float2 z[R1], x[R1];
-            if (!dead) {
-                plast_inv_tw<N, R1, Lay>(z, line, t, wk, wre, wim);
-            } else {
+            for (int t = pt; t < S1; t += 2 * TPL) {
+                float2 wre[R1], wim[R1];
+                load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
+                float4 xx[R1];
 #pragma unroll
-                for (int j = 0; j < R1; ++j) z[j] = make_float2(0.f, 0.f);
-            }
+                for (int j = 0; j < R1; ++j) {
+                    const int r = t + j * S1;
+                    xx[j] = stg[r * CPR + ((l0 >> 1) ^ swz(r))];
+                }
+                float2 z0[R1], z1[R1], x[R1];
+                if (!dp[0]) {
+                    plast_inv_tw<N, R1, Lay>(z0, l0, t, wk, wre, wim);
+                } else {
 #pragma unroll
-            for (int j = 0; j < R1; ++j) {
-                float2 &e = io_at(t + j * S1);
-                x[j] = e;
-                e = z[j];
+                    for (int j = 0; j < R1; ++j) z0[j] = make_float2(0.f, 0.f);
+                }
+                if (more && !dn[0]) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) x[j] = make_float2(xx[j].x, xx[j].y);
+                    pfirst_fwd_tw<N, R1, Lay>(x, l0, t, wk, wre, wim);
+                }
+                if (!dp[1]) {
+                    plast_inv_tw<N, R1, Lay>(z1, l0 + 1, t, wk, wre, wim);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) z1[j] = make_float2(0.f, 0.f);
+                }
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const int r = t + j * S1;
+                    stg[r * CPR + ((l0 >> 1) ^ swz(r))] = make_float4(z0[j].x, z0[j].y, z1[j].x, z1[j].y);
+                }
+                if (more && !dn[1]) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) x[j] = make_float2(xx[j].z, xx[j].w);
+                    pfirst_fwd_tw<N, R1, Lay>(x, l0 + 1, t, wk, wre, wim);
+                }
             }
-            if (more && !dead_next) pfirst_fwd_tw<N, R1, Lay>(x, line, t, wk, wre, wim);
+        } else {
+#pragma unroll 1
+            for (int t = lt; t < S1; t += TPL) {
+                float2 wre[R1], wim[R1];
+                load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
+                float2 z[R1], x[R1];
+                if (!dead) {
+                    plast_inv_tw<N, R1, Lay>(z, line, t, wk, wre, wim);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) z[j] = make_float2(0.f, 0.f);
+                }
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    float2 &e = io_at(t + j * S1);
+                    x[j] = e;
+                    e = z[j];
+                }
+                if (more && !dead_next) pfirst_fwd_tw<N, R1, Lay>(x, line, t, wk, wre, wim);
+            }
         }
         fence_async_smem();
         __syncthreads();  // result tile complete, next input consumed, next first stage in place

@@ -2,87 +2,119 @@
 
 namespace {
 
-// Build (once) a CUDA graph holding `batch` terms for frequency f.
-tbs_status build_graph(tbs_plan *pl, Freq &f, int batch, cudaStream_t st) {
-    if (f.graph && f.graph_batch == batch) return TBS_OK;
-    if (f.graph) { cudaGraphExecDestroy(f.graph); f.graph = nullptr; }
+// Build (once) a CUDA graph holding `batch` terms of frequency f on slot `si`; half = 1: grids sized for half of
+// the SMs (two members of a frequency batch share the GPU).
+tbs_status build_graph(tbs_plan *pl, Freq &f, int si, int half, int batch) {
+    TermGraph &tg = f.graph[si][half];
+    if (tg.exec && tg.batch == batch) return TBS_OK;
+    if (tg.exec) { cudaGraphExecDestroy(tg.exec); tg.exec = nullptr; }
     cudaStream_t cs;
     CU(pl, cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     cudaGraph_t g = nullptr;
+    const int sm_limit = half ? (pl->sms + 1) / 2 : 0;
     cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
     if (e == cudaSuccess) {
-        for (int i = 0; i < batch && e == cudaSuccess; ++i) e = launch_term(pl, f, cs);
+        for (int i = 0; i < batch && e == cudaSuccess; ++i) e = launch_term(pl, f, pl->slot[si], cs, sm_limit);
         cudaError_t e2 = cudaStreamEndCapture(cs, &g);
         if (e == cudaSuccess) e = e2;
     }
-    if (e == cudaSuccess) e = cudaGraphInstantiate(&f.graph, g, 0);
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&tg.exec, g, 0);
     if (g) cudaGraphDestroy(g);
     cudaStreamDestroy(cs);
-    (void)st;
-    if (e != cudaSuccess) { f.graph = nullptr; return fail(pl, TBS_ERR_CUDA, "graph build: %s", cudaGetErrorString(e)); }
-    f.graph_batch = batch;
+    if (e != cudaSuccess) { tg.exec = nullptr; return fail(pl, TBS_ERR_CUDA, "graph build: %s", cudaGetErrorString(e)); }
+    tg.batch = batch;
     return TBS_OK;
 }
 
-// Run the series for one frequency.  The field is left in f.p, history in pl->h_hist.
-tbs_status solve_one(tbs_plan *pl, int ifreq, int max_terms, double tol, cudaStream_t st, int *n_terms_out) {
+// One series in flight on a slot: term 0, then batches of terms with the stop flag read back double-buffered
+// (batch i+1 is enqueued before the flag of batch i is looked at).
+struct Run {
+    int ifreq = -1;
+    int si = 0;
+    cudaStream_t st = nullptr;
+    int half = 0;
+    int issued = 0;      // batches enqueued
+    int checked = 0;     // batches whose flag has been read
+    int max_batches = 0;
+    bool active = false;
+};
+
+tbs_status run_begin(tbs_plan *pl, Run &r, int ifreq, int si, cudaStream_t st, int half, int max_terms, double tol) {
     Freq &f = pl->fr[ifreq];
+    Slot &s = pl->slot[si];
     if (!f.have_V) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_medium / tbs_set_potential not called");
     if (!f.have_S) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_source / tbs_set_source_field not called");
-    tbs_status hs = ensure_history(pl, max_terms);
-    if (hs != TBS_OK) return hs;
     const int batch = pl->graph_batch > 0 ? pl->graph_batch : 8;
-    if (pl->graph_batch > 0) {
-        tbs_status gs = build_graph(pl, f, batch, st);
-        if (gs != TBS_OK) return gs;
-    }
-    Ctl *h = pl->h_ctl;
+    r = Run();
+    r.ifreq = ifreq; r.si = si; r.st = st; r.half = half; r.active = true;
+    r.max_batches = (max_terms + 1 + batch - 1) / batch + 1;
+    Ctl *h = s.h_ctl;
     memset(&h[0], 0, sizeof(Ctl));
     h[0].max_terms = max_terms;
     h[0].tol = tol;
     h[0].status = 1;
     CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
-    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * (max_terms + 1), st));
-    CU(pl, cudaMemsetAsync(pl->history, 0, sizeof(double) * (max_terms + 1), st));
-    CU(pl, cudaEventRecord(pl->ev_t0, st));
+    CU(pl, cudaMemsetAsync(s.norms, 0, sizeof(double) * 2 * (max_terms + 1), st));
+    CU(pl, cudaMemsetAsync(s.history, 0, sizeof(double) * (max_terms + 1), st));
+    CU(pl, cudaEventRecord(s.ev_t0, st));
     // term 0 forward half: W = FFT_x(pad(S / k0^2))
-    RowArgs r;
-    fill_row_args(pl, f, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
-    CU(pl, launch_row<true>(pl->n[0], r, st));
+    RowArgs ra;
+    fill_row_args(pl, f, s, ra, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row(pl->n[0], true, ra, st, false, half ? (pl->sms + 1) / 2 : 0));
     pl->launches += 1;
-    const int per_term = mid_launches(pl) + 1;
-    // batches, double-buffered: enqueue batch i+1 before looking at the flag of batch i
-    int issued = 0;
-    bool done = false;
-    const int max_batches = (max_terms + 1 + batch - 1) / batch + 1;
-    for (int b = 0; b < max_batches + 1 && !done; ++b) {
-        if (b < max_batches) {
-            if (pl->graph_batch > 0) {
-                CU(pl, cudaGraphLaunch(f.graph, st));
-            } else {
-                for (int i = 0; i < batch; ++i) CU(pl, launch_term(pl, f, st));
-            }
-            pl->launches += (long long)batch * per_term;
-            CU(pl, cudaMemcpyAsync(&h[1 + (b & 1)], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
-            CU(pl, cudaEventRecord(pl->ev[b & 1], st));
-            ++issued;
-        }
-        if (b >= 1) {
-            CU(pl, cudaEventSynchronize(pl->ev[(b - 1) & 1]));
-            if (h[1 + ((b - 1) & 1)].done) done = true;
-        }
+    return TBS_OK;
+}
+
+// Enqueue one more batch of terms (and the read-back of the flag behind it).
+tbs_status run_enqueue(tbs_plan *pl, Run &r) {
+    Freq &f = pl->fr[r.ifreq];
+    Slot &s = pl->slot[r.si];
+    const int batch = pl->graph_batch > 0 ? pl->graph_batch : 8;
+    if (pl->graph_batch > 0) {
+        tbs_status gs = build_graph(pl, f, r.si, r.half, batch);
+        if (gs != TBS_OK) return gs;
+        CU(pl, cudaGraphLaunch(f.graph[r.si][r.half].exec, r.st));
+    } else {
+        for (int i = 0; i < batch; ++i) CU(pl, launch_term(pl, f, s, r.st, r.half ? (pl->sms + 1) / 2 : 0));
     }
-    CU(pl, cudaEventRecord(pl->ev_t1, st));
-    CU(pl, cudaMemcpyAsync(&h[3], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
-    CU(pl, cudaMemcpyAsync(pl->h_hist, pl->history, sizeof(double) * (max_terms + 1), cudaMemcpyDeviceToHost, st));
-    CU(pl, cudaStreamSynchronize(st));
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, pl->ev_t0, pl->ev_t1);
-    pl->loop_ms += ms;
-    if (!h[3].done) return fail(pl, TBS_ERR_CUDA, "term loop ended without the stop flag (issued %d batches)", issued);
-    *n_terms_out = h[3].n_terms;
-    if (h[3].status == TBS_ERR_DIVERGED) fail(pl, TBS_ERR_DIVERGED, "term norm became non-finite at term %d", h[3].n_terms);
-    return (tbs_status)h[3].status;
+    pl->launches += (long long)batch * (mid_launches(pl) + 1);
+    CU(pl, cudaMemcpyAsync(&s.h_ctl[1 + (r.issued & 1)], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, r.st));
+    CU(pl, cudaEventRecord(s.ev[r.issued & 1], r.st));
+    ++r.issued;
+    return TBS_OK;
+}
+
+// Wait for the oldest unchecked batch; *done = its stop flag.
+tbs_status run_check(tbs_plan *pl, Run &r, bool *done) {
+    Slot &s = pl->slot[r.si];
+    CU(pl, cudaEventSynchronize(s.ev[r.checked & 1]));
+    *done = s.h_ctl[1 + (r.checked & 1)].done != 0;
+    ++r.checked;
+    return TBS_OK;
+}
+
+// The series has stopped: copy the field and the history out; the slot is free afterwards.
+tbs_status run_finish(tbs_plan *pl, Run &r, int max_terms, float *p_out, bool out_is_host, double *history,
+                      int32_t *n_terms, tbs_status *status) {
+    Freq &f = pl->fr[r.ifreq];
+    Slot &s = pl->slot[r.si];
+    CU(pl, cudaEventRecord(s.ev_t1, r.st));
+    CU(pl, cudaMemcpyAsync(&s.h_ctl[3], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, r.st));
+    CU(pl, cudaMemcpyAsync(s.h_hist, s.history, sizeof(double) * (max_terms + 1), cudaMemcpyDeviceToHost, r.st));
+    CU(pl, cudaMemcpyAsync((float2 *)p_out + (size_t)r.ifreq * pl->npts, f.p, sizeof(float2) * pl->npts,
+                           out_is_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, r.st));
+    CU(pl, cudaStreamSynchronize(r.st));
+    r.active = false;
+    const Ctl &c = s.h_ctl[3];
+    if (!c.done) return fail(pl, TBS_ERR_CUDA, "term loop ended without the stop flag (issued %d batches)", r.issued);
+    n_terms[r.ifreq] = c.n_terms;
+    double *hrow = history + (size_t)r.ifreq * (max_terms + 1);
+    for (int k = 0; k <= max_terms; ++k) hrow[k] = k <= c.n_terms ? s.h_hist[k] : 0.0;
+    if (c.status == TBS_ERR_DIVERGED)
+        fail(pl, TBS_ERR_DIVERGED, "series diverged at term %d of frequency %d (non-finite or growing term norm, PAPER.md:158)",
+             c.n_terms, r.ifreq);
+    *status = (tbs_status)c.status;
+    return TBS_OK;
 }
 
 tbs_status worst(tbs_status a, tbs_status b) {
@@ -91,24 +123,87 @@ tbs_status worst(tbs_status a, tbs_status b) {
     return a > b ? a : b;
 }
 
+// All frequencies of the plan.  One frequency: the series runs on the caller's stream on slot 0.  Several: up to
+// `concurrency` members are in flight at once, each on its slot's own stream with grids sized for its share of the
+// SMs, so that the HBM-bound passes of one member overlap the FP32-bound convolution pass of another; a member that
+// has converged hands its slot to the next frequency, the last one alone goes back to full-width grids.
 tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool out_is_host,
                      double *history, int32_t *n_terms, cudaStream_t st) {
     if (!pl || max_terms < 0 || !(tol >= 0) || !p_out || !history || !n_terms) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     pl->launches = 0;
     pl->loop_ms = 0;
+    tbs_status hs = ensure_history(pl, max_terms);
+    if (hs != TBS_OK) return hs;
+    const int nf = (int)pl->fr.size();
+    const int conc = nf > 1 ? (pl->concurrency < pl->nslots ? pl->concurrency : pl->nslots) : 1;
     tbs_status res = TBS_OK;
-    for (int i = 0; i < (int)pl->fr.size(); ++i) {
-        int nt = 0;
-        tbs_status s = solve_one(pl, i, max_terms, tol, st, &nt);
-        if (s < 0 && s != TBS_ERR_DIVERGED) return s;
-        n_terms[i] = nt;
-        double *hrow = history + (size_t)i * (max_terms + 1);
-        for (int k = 0; k <= max_terms; ++k) hrow[k] = k <= nt ? pl->h_hist[k] : 0.0;
-        CU(pl, cudaMemcpyAsync((float2 *)p_out + (size_t)i * pl->npts, pl->fr[i].p, sizeof(float2) * pl->npts,
-                               out_is_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
-        res = worst(res, s);
+    Run run[kMaxSlots];
+    int next = 0, live = 0;
+    const bool forked = conc > 1;
+    CU(pl, cudaEventRecord(pl->ev_b0, st));
+    if (forked) {
+        CU(pl, cudaEventRecord(pl->ev_fork, st));
+        for (int i = 0; i < conc; ++i) CU(pl, cudaStreamWaitEvent(pl->slot[i].own_stream, pl->ev_fork, 0));
     }
+    auto start_next = [&](int si) -> tbs_status {
+        if (next >= nf) return TBS_OK;
+        const int half = forked && (live + 1 > 1 || nf - next > 1) ? 1 : 0;
+        tbs_status s = run_begin(pl, run[si], next, si, forked ? pl->slot[si].own_stream : st, half, max_terms, tol);
+        if (s == TBS_OK) { ++next; ++live; }
+        return s;
+    };
+    for (int i = 0; i < conc; ++i) {
+        tbs_status s = start_next(i);
+        if (s != TBS_OK) return s;
+    }
+    while (live > 0) {
+        // keep two batches in flight on every live slot, then look at the oldest flag of each
+        for (int i = 0; i < conc; ++i) {
+            Run &r = run[i];
+            while (r.active && r.issued - r.checked < 2 && r.issued < r.max_batches) {
+                if (forked && live == 1 && next >= nf) r.half = 0;   // alone: full-width grids from here on
+                tbs_status s = run_enqueue(pl, r);
+                if (s != TBS_OK) return s;
+            }
+        }
+        for (int i = 0; i < conc; ++i) {
+            Run &r = run[i];
+            if (!r.active) continue;
+            if (r.checked >= r.issued) return fail(pl, TBS_ERR_CUDA, "term loop ran out of batches without the stop flag");
+            bool done = false;
+            tbs_status s = run_check(pl, r, &done);
+            if (s != TBS_OK) return s;
+            if (!done) continue;
+            tbs_status sf = TBS_OK;
+            s = run_finish(pl, r, max_terms, p_out, out_is_host, history, n_terms, &sf);
+            if (s != TBS_OK) return s;
+            --live;
+            if (!forked) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, pl->slot[i].ev_t0, pl->slot[i].ev_t1);
+                pl->loop_ms += ms;
+            }
+            if (sf < 0 && sf != TBS_ERR_DIVERGED) return sf;
+            res = worst(res, sf);
+            s = start_next(i);
+            if (s != TBS_OK) return s;
+        }
+    }
+    if (forked) {
+        for (int i = 0; i < conc; ++i) {
+            CU(pl, cudaEventRecord(pl->slot[i].ev_join, pl->slot[i].own_stream));
+            CU(pl, cudaStreamWaitEvent(st, pl->slot[i].ev_join, 0));
+        }
+    }
+    CU(pl, cudaEventRecord(pl->ev_b1, st));
     CU(pl, cudaStreamSynchronize(st));
+    if (forked) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, pl->ev_b0, pl->ev_b1);
+        pl->loop_ms = ms;   // members overlap: device time of the whole batch
+    }
     return res;
 }
 
@@ -128,27 +223,34 @@ tbs_status tbs_solve_host(tbs_plan *pl, int max_terms, double tol, float *p_out_
 
 tbs_status tbs_apply_green(tbs_plan *pl, int ifreq, const float *x, float *out, void *stream) {
     if (!pl || !x || !out || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
     Freq &f = pl->fr[ifreq];
+    Slot &s = pl->slot[0];
     tbs_status hs = ensure_history(pl, 1);
     if (hs != TBS_OK) return hs;
-    // Save the plan's running field: the inverse half writes p.
-    Ctl *h = pl->h_ctl;
+    Ctl *h = s.h_ctl;
     memset(&h[0], 0, sizeof(Ctl));
     h[0].max_terms = 1 << 30;
     h[0].tol = 0.0;
+    h[0].hold = 1;
     CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
-    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
-    // Use `out` itself as the field buffer and a unit window-free pass: A is applied (as in u_0).
+    CU(pl, cudaMemsetAsync(s.norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
+    // `out` itself serves as the field buffer of a window-carrying pass: A is applied (as in u_0).
     RowArgs r;
-    fill_row_args(pl, f, r, (const float2 *)x, (float)(1.0 / (f.k0 * f.k0)), 1);
-    CU(pl, launch_row<true>(pl->n[0], r, st));
-    CU(pl, launch_mid_passes(pl, f, st));
-    fill_row_args(pl, f, r, nullptr, 0.f, 0);
-    r.ucbs = nullptr;  // one plain application of G, whatever the plan's scheme
+    fill_row_args(pl, f, s, r, (const float2 *)x, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row(pl->n[0], true, r, st));
+    KAbs keep = f.kabs;
+    f.kabs = KAbs{0.f, 0.f, 0.f, 0.f};   // one plain application of G, whatever the plan's potential form
+    cudaError_t e = launch_mid_passes(pl, f, s, st);
+    f.kabs = keep;
+    CU(pl, e);
+    fill_row_args(pl, f, s, r, nullptr, 0.f, 0);
+    r.ucbs = nullptr;  // ... and whatever the plan's scheme
     r.p = (float2 *)out;
     r.V = f.V;  // only multiplies a value that is dropped when do_fwd = 0
-    CU(pl, launch_row<false>(pl->n[0], r, st));
+    CU(pl, launch_row(pl->n[0], false, r, st));
     CU(pl, cudaStreamSynchronize(st));
     return TBS_OK;
 }
@@ -167,6 +269,8 @@ tbs_status tbs_solve_harmonics(tbs_plan *const *plans, int n_harm, int max_terms
             if (p1->n[a] != ph->n[a]) return fail(ph, TBS_ERR_INVALID_ARG, "plans differ in grid size");
         if (fabs(ph->fr[0].f - (h + 1) * p1->fr[0].f) > 1e-9 * p1->fr[0].f)
             return fail(ph, TBS_ERR_INVALID_ARG, "plan %d must be created at %d times the fundamental", h, h + 1);
+        tbs_status ws = ensure_workspace(ph);
+        if (ws != TBS_OK) return ws;
     }
     const int nslow = p1->ndim == 2 ? p1->n[1] : p1->n[2];
     if (ref_row < 0 || ref_row >= nslow) return fail(p1, TBS_ERR_INVALID_ARG, "ref_row outside the grid");
@@ -176,8 +280,12 @@ tbs_status tbs_solve_harmonics(tbs_plan *const *plans, int n_harm, int max_terms
     if (res < 0) return res;
     if (surface_pressure_pa > 0.0) {
         const long long slab = n / nslow;
-        cudaMemsetAsync(p1->maxbits, 0, sizeof(unsigned int), st);
+        CU(p1, cudaMemsetAsync(p1->maxbits, 0, sizeof(unsigned int), st));
         k_row_max<<<nblk(slab, 256), 256, 0, st>>>(p1->fr[0].p, (long long)ref_row * slab, slab, p1->maxbits);
+        unsigned int bits = 0;
+        CU(p1, cudaMemcpyAsync(&bits, p1->maxbits, sizeof bits, cudaMemcpyDeviceToHost, st));
+        CU(p1, cudaStreamSynchronize(st));
+        if (bits == 0u) return fail(p1, TBS_ERR_INVALID_ARG, "the fundamental vanishes on the reference row: nothing to rescale");
         k_rescale_field<<<nblk(n, 256), 256, 0, st>>>(p1->fr[0].p, p1->maxbits, surface_pressure_pa, n);
         CU(p1, cudaGetLastError());
         CU(p1, cudaMemcpyAsync(p_out[0], p1->fr[0].p, sizeof(float2) * n, cudaMemcpyDeviceToDevice, st));
@@ -224,49 +332,48 @@ tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, 
     return s;
 }
 
+// Per-kernel device time of one term.  Each kernel of the term is launched `reps` times back to back between two
+// events on `stream` (so the events cost nothing per launch), after a live series of term 0 and three warm-up
+// terms has put real data in place; the stop logic is held off (Ctl::hold), since a pass repeated on its own
+// output may overflow -- which does not change what a launch costs.
 tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4], void *stream) {
     if (!pl || !out_ms || reps < 1 || reps > 256 || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     Freq &f = pl->fr[ifreq];
+    Slot &s = pl->slot[0];
     if (!f.have_V || !f.have_S) return fail(pl, TBS_ERR_NOT_READY, "medium and source required");
     cudaStream_t st = (cudaStream_t)stream;
-    tbs_status hs = ensure_history(pl, reps + 4);
+    tbs_status hs = ensure_history(pl, (reps + 1) * 2 + 8);
     if (hs != TBS_OK) return hs;
-    // A real series: term 0, two warm-up terms, then `reps` terms with an event between kernels.
-    Ctl *h = pl->h_ctl;
+    Ctl *h = s.h_ctl;
     memset(&h[0], 0, sizeof(Ctl));
     h[0].max_terms = 1 << 30;
     h[0].tol = 0.0;
+    h[0].hold = 1;
     CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
-    CU(pl, cudaMemsetAsync(pl->norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
+    CU(pl, cudaMemsetAsync(s.norms, 0, sizeof(double) * 2 * pl->hist_cap, st));
     RowArgs r;
-    fill_row_args(pl, f, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
-    CU(pl, launch_row<true>(pl->n[0], r, st));
-    for (int i = 0; i < 3; ++i) CU(pl, launch_term(pl, f, st));
+    fill_row_args(pl, f, s, r, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
+    CU(pl, launch_row(pl->n[0], true, r, st));
+    for (int i = 0; i < 3; ++i) CU(pl, launch_term(pl, f, s, st));
     const int nmid = mid_launches(pl);
-    const int per = nmid + 1;
-    std::vector<cudaEvent_t> evs((size_t)reps * per + 1);
-    for (auto &e : evs) CU(pl, cudaEventCreate(&e));
-    fill_row_args(pl, f, r, nullptr, 0.f, 1);
-    CU(pl, cudaEventRecord(evs[0], st));
-    for (int i = 0; i < reps; ++i) {
-        for (int k = 0; k < nmid; ++k) {
-            CU(pl, launch_mid_passes(pl, f, st, k));
-            CU(pl, cudaEventRecord(evs[(size_t)i * per + k + 1], st));
-        }
-        CU(pl, launch_row<false>(pl->n[0], r, st));
-        CU(pl, cudaEventRecord(evs[(size_t)i * per + nmid + 1], st));
-    }
-    CU(pl, cudaStreamSynchronize(st));
+    fill_row_args(pl, f, s, r, nullptr, 0.f, 1);
     for (int k = 0; k < 4; ++k) out_ms[k] = 0.0;
-    for (int i = 0; i < reps; ++i)
-        for (int k = 0; k < per; ++k) {
-            float ms = 0.f;
-            cudaEventElapsedTime(&ms, evs[(size_t)i * per + k], evs[(size_t)i * per + k + 1]);
-            // out_ms[0] = row kernel, out_ms[1..] = column/plane passes in launch order
-            out_ms[k == nmid ? 0 : k + 1] += ms / reps;
-        }
-    for (auto &e : evs) cudaEventDestroy(e);
-    return TBS_OK;
+    tbs_status res = TBS_OK;
+    // out_ms[0] = row kernel, out_ms[1..] = column/plane passes in launch order
+    for (int k = 0; k <= nmid && res == TBS_OK; ++k) {
+        cudaError_t e = cudaEventRecord(pl->ev_b0, st);
+        for (int i = 0; i < reps && e == cudaSuccess; ++i)
+            e = k < nmid ? launch_mid_passes(pl, f, s, st, k) : launch_row(pl->n[0], false, r, st);
+        if (e == cudaSuccess) e = cudaEventRecord(pl->ev_b1, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, pl->ev_b0, pl->ev_b1);
+        if (e != cudaSuccess) res = fail(pl, TBS_ERR_CUDA, "tbs_profile_term: %s", cudaGetErrorString(e));
+        out_ms[k == nmid ? 0 : k + 1] = ms / reps;
+    }
+    return res;
 }
 
 }  // extern "C"

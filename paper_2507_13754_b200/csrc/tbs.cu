@@ -17,19 +17,40 @@ using namespace tbs;
 namespace {
 
 constexpr double kPi = 3.14159265358979323846;
+constexpr int kMaxSlots = 2;          // members of a frequency batch in flight at once
+constexpr size_t kWsAlign = 256;      // alignment of every workspace region (TMA / bulk copies need 16)
+
+// A CUDA graph of `batch` Born terms of one frequency on one slot at one grid width.
+struct TermGraph {
+    cudaGraphExec_t exec = nullptr;
+    int batch = 0;
+};
 
 struct Freq {
     double f = 0, omega = 0, k0 = 0;
-    float2 *V = nullptr;      // [n] V/k0^2
-    float2 *S = nullptr;      // [n] source density
-    float2 *p = nullptr;      // [n] running field
+    float2 *V = nullptr;      // [n] V/k0^2                     (workspace)
+    float2 *S = nullptr;      // [n] source density             (workspace)
+    float2 *p = nullptr;      // [n] running field              (workspace)
     float2 *ucbs = nullptr;   // [n] current term of the convergent Born series (allocated by tbs_set_scheme)
     float *p2[3] = {nullptr, nullptr, nullptr};  // per-axis |p|^2/k0^2, position order, [2 n[a]]
     Ctl *ctl = nullptr;
-    cudaGraphExec_t graph = nullptr;
-    int graph_batch = 0;
+    TermGraph graph[kMaxSlots][2];   // [slot][0 = all SMs, 1 = half of them]
     bool have_V = false, have_S = false;
     KAbs kabs = {0.f, 0.f, 0.f, 0.f};  // nu > 0: k-space multiplier potential of Eq. 24 instead of V(r)
+};
+
+// What one series in flight needs beyond its frequency's V, S, p: the transform intermediates, the norm and
+// history buffers, the host mirrors and the events of the batched loop.  Slot 0 serves every single solve;
+// slot 1 exists for plans with more than one frequency (two members of the batch are in flight at once).
+struct Slot {
+    float2 *W1 = nullptr;   // [nz*ny][2 nx]                    (workspace)
+    float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]            (workspace)
+    CUtensorMap conv_map;   // tensor map of the array k_conv transforms in place (W1 in 2-D, W2 in 3-D)
+    double *norms = nullptr, *history = nullptr;   // device, hist_cap entries
+    double *h_hist = nullptr;                      // pinned
+    Ctl *h_ctl = nullptr;                          // pinned, 4 entries
+    cudaStream_t own_stream = nullptr;             // batch members run on the slot's own stream
+    cudaEvent_t ev[2] = {nullptr, nullptr}, ev_t0 = nullptr, ev_t1 = nullptr, ev_join = nullptr;
 };
 
 }  // namespace
@@ -41,27 +62,32 @@ struct tbs_plan {
     double dx = 0, c0 = 0, damping = 0;
     double beta = 1.0, rho0 = 1000.0;
     std::vector<Freq> fr;
+    int nslots = 1;
+    Slot slot[kMaxSlots];
     float2 *lutA[3] = {nullptr, nullptr, nullptr};   // per axis, fft_engine.cuh "Luts"
     float2 *lutB[3] = {nullptr, nullptr, nullptr};
     float2 *lutC[3] = {nullptr, nullptr, nullptr};
     float4 *lutAB[3] = {nullptr, nullptr, nullptr};
-    float2 *W1 = nullptr;   // [nz*ny][2 nx]
-    float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]
-    CUtensorMap conv_map;   // tensor map of the array k_conv transforms in place (W1 in 2-D, W2 in 3-D)
     float *abl[3] = {nullptr, nullptr, nullptr};
-    double *norms = nullptr, *history = nullptr;
+    // workspace: V, S, p of every frequency and W1 (W2) of every slot, in one device range that the caller
+    // may own (tbs_plan_set_workspace) -- otherwise allocated by the plan at first use
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
     int hist_cap = 0;
     unsigned int *maxbits = nullptr;
-    Ctl *h_ctl = nullptr;        // pinned, 4 slots
-    double *h_hist = nullptr;    // pinned staging
-    cudaEvent_t ev[2] = {nullptr, nullptr}, ev_t0 = nullptr, ev_t1 = nullptr;
-    size_t dev_bytes = 0;
+    void *stage = nullptr;       // device staging of tbs_set_source (positions, amplitudes), grows only
+    size_t stage_bytes = 0;
+    cudaEvent_t ev_fork = nullptr, ev_b0 = nullptr, ev_b1 = nullptr;
+    size_t small_bytes = 0;      // device bytes outside the workspace (tables, control)
     int graph_batch = 16;
+    int concurrency = kMaxSlots;
     int scheme = TBS_SCHEME_BORN;
     int boundary = TBS_BOUNDARY_PAD;
     int crit_row = -1;
     long long launches = 0;
     double loop_ms = 0;
+    int sms = 0;
     std::string err;
 };
 
@@ -90,15 +116,76 @@ tbs_status fail(tbs_plan *p, tbs_status st, const char *fmt, ...) {
 template <class T>
 cudaError_t dmalloc(tbs_plan *p, T **ptr, size_t count) {
     cudaError_t e = cudaMalloc((void **)ptr, count * sizeof(T));
-    if (e == cudaSuccess) p->dev_bytes += count * sizeof(T);
+    if (e == cudaSuccess) p->small_bytes += count * sizeof(T);
     return e;
 }
 
 bool pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 inline unsigned nblk(long long n, int b) { return (unsigned)((n + b - 1) / b); }
+inline size_t align_up(size_t v) { return (v + kWsAlign - 1) / kWsAlign * kWsAlign; }
 
-void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float src_scale, int do_fwd) {
-    a.W = pl->W1;
+size_t w1_elems(const tbs_plan *pl) { return (size_t)pl->n[1] * pl->n[2] * 2 * pl->n[0]; }
+size_t w2_elems(const tbs_plan *pl) { return pl->ndim == 3 ? (size_t)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0] : 0; }
+
+// Layout of the workspace: V, S, p of frequency 0, 1, ...; then W1 (and W2) of slot 0, 1.
+size_t workspace_layout(tbs_plan *pl, char *base, bool bind) {
+    size_t off = 0;
+    auto take = [&](size_t elems) {
+        float2 *ptr = bind ? reinterpret_cast<float2 *>(base + off) : nullptr;
+        off += align_up(elems * sizeof(float2));
+        return ptr;
+    };
+    for (auto &f : pl->fr) {
+        float2 *v = take((size_t)pl->npts), *s = take((size_t)pl->npts), *p = take((size_t)pl->npts);
+        if (bind) { f.V = v; f.S = s; f.p = p; }
+    }
+    for (int i = 0; i < pl->nslots; ++i) {
+        float2 *w1 = take(w1_elems(pl));
+        float2 *w2 = pl->ndim == 3 ? take(w2_elems(pl)) : nullptr;
+        if (bind) { pl->slot[i].W1 = w1; pl->slot[i].W2 = w2; }
+    }
+    return off;
+}
+
+void destroy_graphs(tbs_plan *pl) {
+    for (auto &f : pl->fr)
+        for (auto &row : f.graph)
+            for (auto &g : row) {
+                if (g.exec) cudaGraphExecDestroy(g.exec);
+                g.exec = nullptr;
+                g.batch = 0;
+            }
+}
+
+// Point the plan at a workspace.  Its contents are undefined: medium and source have to be set (again).
+tbs_status bind_workspace(tbs_plan *pl, void *base, size_t bytes, bool owned) {
+    destroy_graphs(pl);
+    if (pl->ws && pl->ws_owned) cudaFree(pl->ws);
+    pl->ws = base;
+    pl->ws_bytes = bytes;
+    pl->ws_owned = owned;
+    workspace_layout(pl, (char *)base, true);
+    for (auto &f : pl->fr) { f.have_V = false; f.have_S = false; }
+    const long long mx = 2LL * pl->n[0], my = 2LL * pl->n[1];
+    for (int i = 0; i < pl->nslots; ++i) {
+        Slot &s = pl->slot[i];
+        if (pl->ndim == 2) CU(pl, make_conv_tensor_map(&s.conv_map, s.W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
+        else CU(pl, make_conv_tensor_map(&s.conv_map, s.W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
+    }
+    return TBS_OK;
+}
+
+// Every call that touches V, S, p or W goes through here: without a caller-owned workspace the plan allocates.
+tbs_status ensure_workspace(tbs_plan *pl) {
+    if (pl->ws) return TBS_OK;
+    const size_t bytes = workspace_layout(pl, nullptr, false);
+    void *base = nullptr;
+    CU(pl, cudaMalloc(&base, bytes));
+    return bind_workspace(pl, base, bytes, true);
+}
+
+void fill_row_args(tbs_plan *pl, Freq &f, Slot &s, RowArgs &a, const float2 *src, float src_scale, int do_fwd) {
+    a.W = s.W1;
     a.src = src;
     a.V = f.V;
     a.p = f.p;
@@ -114,14 +201,14 @@ void fill_row_args(tbs_plan *pl, Freq &f, RowArgs &a, const float2 *src, float s
     a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
     if (pl->boundary == TBS_BOUNDARY_PERIODIC) a.scale *= (float)(1 << pl->ndim);  // the odd half carries nothing
     a.do_fwd = do_fwd;
-    a.norms = pl->norms;
-    a.history = pl->history;
+    a.norms = s.norms;
+    a.history = s.history;
     a.ctl = f.ctl;
     a.lut = Luts{pl->lutA[0], pl->lutB[0], pl->lutC[0], pl->lutAB[0]};
 }
 
 // Column / plane passes of one term (K2 in 2-D; y-forward, z-conv, y-inverse in 3-D).
-cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which = -1) {
+cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int which = -1, int sm_limit = 0) {
     const int nx = pl->n[0], ny = pl->n[1], nz = pl->n[2];
     const long long mx = 2LL * nx, my = 2LL * ny;
     ColArgs a;
@@ -133,56 +220,56 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, cudaStream_t st, int which 
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
-        a.in = pl->W1; a.out = pl->W1;
+        a.in = s.W1; a.out = s.W1;
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = a.out_line_stride = mx;
         a.p2_line = (const float2 *)f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
-        if (which < 0 || which == 0) e = launch_conv(ny, a, &pl->conv_map, 1, st);
+        if (which < 0 || which == 0) e = launch_conv(ny, a, &s.conv_map, 1, st, false, sm_limit);
         return e;
     }
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
     if (which < 0 || which == 0) {
-        a.in = pl->W1; a.out = pl->W2;
+        a.in = s.W1; a.out = s.W2;
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = (long long)ny * mx; a.out_outer_stride = my * mx;
-        e = launch_col<MODE_FWD>(ny, a, nz, st);
+        e = launch_col(ny, MODE_FWD, a, nz, st, false, sm_limit);
         if (e != cudaSuccess) return e;
     }
     // z convolution, in place on W2; lines (ky, kx), outer = ky
     if (which < 0 || which == 1) {
-        a.in = pl->W2; a.out = pl->W2;
+        a.in = s.W2; a.out = s.W2;
         a.lut = Luts{pl->lutA[2], pl->lutB[2], pl->lutC[2], pl->lutAB[2]};
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
         a.p2_line = (const float2 *)f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
-        e = launch_conv(nz, a, &pl->conv_map, (int)my, st);
+        e = launch_conv(nz, a, &s.conv_map, (int)my, st, false, sm_limit);
         if (e != cudaSuccess) return e;
     }
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
     if (which < 0 || which == 2) {
-        a.in = pl->W2; a.out = pl->W1;
+        a.in = s.W2; a.out = s.W1;
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = my * mx; a.out_outer_stride = (long long)ny * mx;
         a.p2_line = nullptr; a.p2_inner = nullptr; a.p2_outer = nullptr;
-        e = launch_col<MODE_INV>(ny, a, nz, st);
+        e = launch_col(ny, MODE_INV, a, nz, st, false, sm_limit);
     }
     return e;
 }
 
 int mid_launches(const tbs_plan *pl) { return pl->ndim == 2 ? 1 : 3; }
 
-cudaError_t launch_term(tbs_plan *pl, Freq &f, cudaStream_t st, int do_fwd = 1) {
-    cudaError_t e = launch_mid_passes(pl, f, st);
+cudaError_t launch_term(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int sm_limit = 0) {
+    cudaError_t e = launch_mid_passes(pl, f, s, st, -1, sm_limit);
     if (e != cudaSuccess) return e;
     RowArgs r;
-    fill_row_args(pl, f, r, nullptr, 0.f, do_fwd);
-    return launch_row<false>(pl->n[0], r, st);
+    fill_row_args(pl, f, s, r, nullptr, 0.f, 1);
+    return launch_row(pl->n[0], false, r, st, false, sm_limit);
 }
 
 // Green's-spectrum axis tables of one frequency, in the order each kernel reads them (setup_kernels.cuh).
-void fill_axis_tables(tbs_plan *pl, Freq &f) {
+cudaError_t fill_axis_tables(tbs_plan *pl, Freq &f) {
     for (int a = 0; a < pl->ndim; ++a) {
         int r1, r2, rl;
         radices_of(pl->n[a], r1, r2, rl);
@@ -191,49 +278,85 @@ void fill_axis_tables(tbs_plan *pl, Freq &f) {
                                                         a == pl->ndim - 1 ? 1.0 / pl->damping : 1.0,
                                                         pl->boundary == TBS_BOUNDARY_PERIODIC);
     }
+    return cudaGetLastError();
 }
 
 cudaError_t set_kernel_attrs(tbs_plan *pl) {
     ColArgs ca; memset(&ca, 0, sizeof ca);
     RowArgs ra; memset(&ra, 0, sizeof ra);
     cudaError_t e;
-    if ((e = launch_row<true>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
-    if ((e = launch_row<false>(pl->n[0], ra, 0, true)) != cudaSuccess) return e;
+    if ((e = launch_row(pl->n[0], true, ra, 0, true)) != cudaSuccess) return e;
     if (pl->ndim == 2) return launch_conv(pl->n[1], ca, nullptr, 1, 0, true);
-    if ((e = launch_col<MODE_FWD>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
-    if ((e = launch_col<MODE_INV>(pl->n[1], ca, 1, 0, true)) != cudaSuccess) return e;
+    if ((e = launch_col(pl->n[1], MODE_FWD, ca, 1, 0, true)) != cudaSuccess) return e;
     return launch_conv(pl->n[2], ca, nullptr, 1, 0, true);
 }
 
+// Norm and history buffers of every slot for series of up to max_terms terms.  The captured graphs hold these
+// pointers, so a reallocation drops the graphs.
 tbs_status ensure_history(tbs_plan *pl, int max_terms) {
     if (max_terms + 1 <= pl->hist_cap) return TBS_OK;
-    if (pl->norms) { cudaFree(pl->norms); cudaFree(pl->history); cudaFreeHost(pl->h_hist); }
-    pl->norms = nullptr; pl->history = nullptr; pl->h_hist = nullptr;
+    destroy_graphs(pl);
     const int cap = max_terms + 1;
-    CU(pl, cudaMalloc((void **)&pl->norms, sizeof(double) * 2 * cap));
-    CU(pl, cudaMalloc((void **)&pl->history, sizeof(double) * cap));
-    CU(pl, cudaMallocHost((void **)&pl->h_hist, sizeof(double) * cap));
+    for (int i = 0; i < pl->nslots; ++i) {
+        Slot &s = pl->slot[i];
+        if (s.norms) cudaFree(s.norms);
+        if (s.history) cudaFree(s.history);
+        if (s.h_hist) cudaFreeHost(s.h_hist);
+        s.norms = nullptr; s.history = nullptr; s.h_hist = nullptr;
+        pl->hist_cap = 0;
+        CU(pl, cudaMalloc((void **)&s.norms, sizeof(double) * 2 * cap));
+        CU(pl, cudaMalloc((void **)&s.history, sizeof(double) * cap));
+        CU(pl, cudaMallocHost((void **)&s.h_hist, sizeof(double) * cap));
+    }
     pl->hist_cap = cap;
     return TBS_OK;
 }
 
-void destroy_graphs(tbs_plan *pl) {
-    for (auto &f : pl->fr) {
-        if (f.graph) cudaGraphExecDestroy(f.graph);
-        f.graph = nullptr;
-        f.graph_batch = 0;
-    }
+// Grow-only device staging buffer (tbs_set_source).
+tbs_status ensure_stage(tbs_plan *pl, size_t bytes) {
+    if (bytes <= pl->stage_bytes) return TBS_OK;
+    if (pl->stage) cudaFree(pl->stage);
+    pl->stage = nullptr;
+    pl->stage_bytes = 0;
+    const size_t cap = bytes < 65536 ? 65536 : bytes * 2;
+    CU(pl, cudaMalloc(&pl->stage, cap));
+    pl->stage_bytes = cap;
+    return TBS_OK;
 }
 
 }  // namespace
 
 extern "C" {
 
-const char *tbs_version(void) { return "tbs-b200 0.1 (sm_100a)"; }
+const char *tbs_version(void) { return "tbs-b200 0.2 (sm_100a)"; }
 
 const char *tbs_last_error(const tbs_plan *plan) { return plan ? plan->err.c_str() : "null plan"; }
 
-size_t tbs_plan_workspace_bytes(const tbs_plan *plan) { return plan ? plan->dev_bytes : 0; }
+size_t tbs_plan_workspace_bytes(const tbs_plan *plan) {
+    return plan ? workspace_layout(const_cast<tbs_plan *>(plan), nullptr, false) : 0;
+}
+
+tbs_status tbs_plan_set_workspace(tbs_plan *pl, void *dev_ptr, size_t bytes) {
+    if (!pl || !dev_ptr) return TBS_ERR_INVALID_ARG;
+    if (((uintptr_t)dev_ptr % kWsAlign) != 0) return fail(pl, TBS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    const size_t need = workspace_layout(pl, nullptr, false);
+    if (bytes < need) return fail(pl, TBS_ERR_INVALID_ARG, "workspace of %zu bytes, %zu needed", bytes, need);
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, dev_ptr) != cudaSuccess || at.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return fail(pl, TBS_ERR_INVALID_ARG, "workspace is not device memory");
+    }
+    CU(pl, cudaDeviceSynchronize());
+    return bind_workspace(pl, dev_ptr, bytes, false);
+}
+
+size_t tbs_plan_device_bytes(const tbs_plan *plan) {
+    return plan ? plan->small_bytes + (plan->ws_owned ? plan->ws_bytes : 0) : 0;
+}
+
+double tbs_grid_harmonic_frequency(int m, double c0, int n, double dx_m) {
+    return (m > 0 && n > 0 && dx_m > 0 && c0 > 0) ? (double)m * c0 / ((double)n * dx_m) : 0.0;
+}
 
 int64_t tbs_last_launch_count(const tbs_plan *plan) { return plan ? plan->launches : 0; }
 double tbs_last_loop_ms(const tbs_plan *plan) { return plan ? plan->loop_ms : 0.0; }
@@ -245,22 +368,38 @@ tbs_status tbs_set_graph_batch(tbs_plan *plan, int terms_per_graph) {
     return TBS_OK;
 }
 
+tbs_status tbs_set_concurrency(tbs_plan *plan, int members) {
+    if (!plan || members < 1 || members > kMaxSlots) return TBS_ERR_INVALID_ARG;
+    plan->concurrency = members;
+    return TBS_OK;
+}
+
 void tbs_plan_destroy(tbs_plan *pl) {
     if (!pl) return;
+    cudaDeviceSynchronize();
     destroy_graphs(pl);
     for (auto &f : pl->fr) {
-        cudaFree(f.V); cudaFree(f.S); cudaFree(f.p); cudaFree(f.ctl); cudaFree(f.ucbs);
+        cudaFree(f.ctl); cudaFree(f.ucbs);
         for (int a = 0; a < 3; ++a) cudaFree(f.p2[a]);
     }
+    if (pl->ws && pl->ws_owned) cudaFree(pl->ws);
     for (int a = 0; a < 3; ++a) { cudaFree(pl->lutA[a]); cudaFree(pl->lutB[a]); cudaFree(pl->lutC[a]); cudaFree(pl->lutAB[a]); }
-    cudaFree(pl->W1); cudaFree(pl->W2);
     for (int a = 0; a < 3; ++a) cudaFree(pl->abl[a]);
-    cudaFree(pl->norms); cudaFree(pl->history); cudaFree(pl->maxbits);
-    if (pl->h_ctl) cudaFreeHost(pl->h_ctl);
-    if (pl->h_hist) cudaFreeHost(pl->h_hist);
-    for (int i = 0; i < 2; ++i) if (pl->ev[i]) cudaEventDestroy(pl->ev[i]);
-    if (pl->ev_t0) cudaEventDestroy(pl->ev_t0);
-    if (pl->ev_t1) cudaEventDestroy(pl->ev_t1);
+    cudaFree(pl->maxbits);
+    cudaFree(pl->stage);
+    for (auto &s : pl->slot) {
+        cudaFree(s.norms); cudaFree(s.history);
+        if (s.h_ctl) cudaFreeHost(s.h_ctl);
+        if (s.h_hist) cudaFreeHost(s.h_hist);
+        for (int i = 0; i < 2; ++i) if (s.ev[i]) cudaEventDestroy(s.ev[i]);
+        if (s.ev_t0) cudaEventDestroy(s.ev_t0);
+        if (s.ev_t1) cudaEventDestroy(s.ev_t1);
+        if (s.ev_join) cudaEventDestroy(s.ev_join);
+        if (s.own_stream) cudaStreamDestroy(s.own_stream);
+    }
+    if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
+    if (pl->ev_b0) cudaEventDestroy(pl->ev_b0);
+    if (pl->ev_b1) cudaEventDestroy(pl->ev_b1);
     delete pl;
 }
 
@@ -284,8 +423,12 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
     pl->npts = (long long)pl->n[0] * pl->n[1] * pl->n[2];
     pl->dx = dx_m; pl->c0 = c0; pl->damping = damping;
     pl->fr.resize(nfreq);
+    pl->nslots = nfreq > 1 ? kMaxSlots : 1;
     tbs_status st = TBS_OK;
     auto build = [&]() -> tbs_status {
+        int dev = 0;
+        CU(pl, cudaGetDevice(&dev));
+        CU(pl, cudaDeviceGetAttribute(&pl->sms, cudaDevAttrMultiProcessorCount, dev));
         CU(pl, set_kernel_attrs(pl));
         for (int a = 0; a < ndim; ++a) {
             int r1, r2, rl;
@@ -301,35 +444,34 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
                 CU(pl, dmalloc(pl, &pl->lutC[a], N / r1));
                 k_stage_lut<<<nblk(N / r1, 256), 256>>>(pl->lutC[a], N / r1, r2, 0);
             }
-        }
-        const long long rows = (long long)pl->n[1] * pl->n[2];
-        CU(pl, dmalloc(pl, &pl->W1, (size_t)(rows * 2 * pl->n[0])));
-        if (ndim == 3) CU(pl, dmalloc(pl, &pl->W2, (size_t)((long long)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0])));
-        {
-            const long long mx = 2LL * pl->n[0], my = 2LL * pl->n[1];
-            if (ndim == 2) CU(pl, make_conv_tensor_map(&pl->conv_map, pl->W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
-            else CU(pl, make_conv_tensor_map(&pl->conv_map, pl->W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
+            CU(pl, cudaGetLastError());
         }
         for (int a = 0; a < ndim; ++a) {
             CU(pl, dmalloc(pl, &pl->abl[a], pl->n[a]));
             k_abl_window<<<nblk(pl->n[a], 256), 256>>>(pl->abl[a], pl->n[a], 0, 0.0);
         }
+        CU(pl, cudaGetLastError());
         CU(pl, dmalloc(pl, &pl->maxbits, 1));
-        CU(pl, cudaMallocHost((void **)&pl->h_ctl, sizeof(Ctl) * 4));
-        for (int i = 0; i < 2; ++i) CU(pl, cudaEventCreateWithFlags(&pl->ev[i], cudaEventDisableTiming));
-        CU(pl, cudaEventCreate(&pl->ev_t0));
-        CU(pl, cudaEventCreate(&pl->ev_t1));
+        for (int i = 0; i < pl->nslots; ++i) {
+            Slot &s = pl->slot[i];
+            CU(pl, cudaMallocHost((void **)&s.h_ctl, sizeof(Ctl) * 4));
+            for (int k = 0; k < 2; ++k) CU(pl, cudaEventCreateWithFlags(&s.ev[k], cudaEventDisableTiming));
+            CU(pl, cudaEventCreate(&s.ev_t0));
+            CU(pl, cudaEventCreate(&s.ev_t1));
+            CU(pl, cudaEventCreateWithFlags(&s.ev_join, cudaEventDisableTiming));
+            if (pl->nslots > 1) CU(pl, cudaStreamCreateWithFlags(&s.own_stream, cudaStreamNonBlocking));
+        }
+        CU(pl, cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+        CU(pl, cudaEventCreate(&pl->ev_b0));
+        CU(pl, cudaEventCreate(&pl->ev_b1));
         for (int i = 0; i < nfreq; ++i) {
             Freq &f = pl->fr[i];
             f.f = f_hz[i];
             f.omega = 2.0 * kPi * f.f;
             f.k0 = f.omega / c0;
-            CU(pl, dmalloc(pl, &f.V, (size_t)pl->npts));
-            CU(pl, dmalloc(pl, &f.S, (size_t)pl->npts));
-            CU(pl, dmalloc(pl, &f.p, (size_t)pl->npts));
             CU(pl, dmalloc(pl, &f.ctl, 1));
             for (int a = 0; a < ndim; ++a) CU(pl, dmalloc(pl, &f.p2[a], 2 * pl->n[a]));
-            fill_axis_tables(pl, f);
+            CU(pl, fill_axis_tables(pl, f));
         }
         CU(pl, cudaDeviceSynchronize());
         return TBS_OK;
@@ -354,10 +496,14 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
     if (!pl || !(alpha0_si >= 0.0)) return TBS_ERR_INVALID_ARG;
     if (alpha0_si > 0.0 && (!(nu > 0.0) || nu > 2.0 || fabs(nu - 1.0) < 1e-9))
         return fail(pl, TBS_ERR_INVALID_ARG, "power-law exponent must lie in (0, 2] and differ from 1 (PAPER.md:53)");
+    if (alpha0_si > 0.0 && pl->scheme == TBS_SCHEME_CBS)
+        return fail(pl, TBS_ERR_INVALID_ARG, "the k-space multiplier potential is not combined with TBS_SCHEME_CBS");
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     for (auto &f : pl->fr) {
         if (alpha0_si == 0.0) {
+            if (f.kabs.nu > 0.f) f.have_V = false;  // the spatial potential has to be set again
             f.kabs = KAbs{0.f, 0.f, 0.f, 0.f};
-            f.have_V = false;  // the spatial potential has to be set again
             continue;
         }
         // tau = -2 alpha0 v_f^(nu-1), eta = 2 alpha0 v_f^nu tan(pi nu/2)
@@ -371,6 +517,7 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
         f.have_V = true;
     }
     destroy_graphs(pl);
+    CU(pl, cudaGetLastError());
     CU(pl, cudaDeviceSynchronize());
     return TBS_OK;
 }
@@ -378,7 +525,7 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
 tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
     if (!pl || (boundary != TBS_BOUNDARY_PAD && boundary != TBS_BOUNDARY_PERIODIC)) return TBS_ERR_INVALID_ARG;
     pl->boundary = boundary;
-    for (auto &f : pl->fr) fill_axis_tables(pl, f);
+    for (auto &f : pl->fr) CU(pl, fill_axis_tables(pl, f));
     destroy_graphs(pl);  // the captured launches carry the normalisation
     CU(pl, cudaDeviceSynchronize());
     return TBS_OK;
@@ -395,9 +542,13 @@ tbs_status tbs_set_criterion(tbs_plan *pl, int criterion, int row) {
 
 tbs_status tbs_set_scheme(tbs_plan *pl, int scheme) {
     if (!pl || (scheme != TBS_SCHEME_BORN && scheme != TBS_SCHEME_CBS)) return TBS_ERR_INVALID_ARG;
-    if (scheme == TBS_SCHEME_CBS)
+    if (scheme == TBS_SCHEME_CBS) {
+        for (auto &f : pl->fr)
+            if (f.kabs.nu > 0.f)
+                return fail(pl, TBS_ERR_INVALID_ARG, "TBS_SCHEME_CBS is not combined with the k-space multiplier potential");
         for (auto &f : pl->fr)
             if (!f.ucbs) CU(pl, dmalloc(pl, &f.ucbs, (size_t)pl->npts));
+    }
     if (scheme != pl->scheme) destroy_graphs(pl);  // the captured launches carry the scheme
     pl->scheme = scheme;
     return TBS_OK;
@@ -409,8 +560,17 @@ tbs_status tbs_set_abl(tbs_plan *pl, int cells, double zeta_half_mu) {
         if (2 * cells > pl->n[a]) return fail(pl, TBS_ERR_INVALID_ARG, "ABL wider than half the grid");
     for (int a = 0; a < pl->ndim; ++a)
         k_abl_window<<<nblk(pl->n[a], 256), 256>>>(pl->abl[a], pl->n[a], cells, zeta_half_mu);
+    CU(pl, cudaGetLastError());
     CU(pl, cudaDeviceSynchronize());
     return TBS_OK;
+}
+
+// A spatial potential replaces the k-space multiplier of Eq. 24, if one was active (the two are not combined).
+static void drop_kspace_potential(tbs_plan *pl, Freq &f) {
+    if (f.kabs.nu > 0.f) {
+        f.kabs = KAbs{0.f, 0.f, 0.f, 0.f};
+        destroy_graphs(pl);
+    }
 }
 
 tbs_status tbs_set_medium(tbs_plan *pl, const float *c, const float *rho, const float *alpha0_map,
@@ -418,12 +578,15 @@ tbs_status tbs_set_medium(tbs_plan *pl, const float *c, const float *rho, const 
     if (!pl || !c) return TBS_ERR_INVALID_ARG;
     const bool absorbing = alpha0_map != nullptr || alpha0_db != 0.0;
     if (absorbing && fabs(y - 1.0) < 1e-9) return fail(pl, TBS_ERR_INVALID_ARG, "y = 1 is excluded (PAPER.md:53)");
-    if (!(rho0 > 0) && !rho) return fail(pl, TBS_ERR_INVALID_ARG, "rho0 must be positive");
+    if (!(rho0 > 0)) return fail(pl, TBS_ERR_INVALID_ARG, "rho0 must be positive");
     (void)rho;  // density does not enter V; rho0 feeds xi of the harmonic source
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
     pl->beta = beta;
     pl->rho0 = rho0;
     for (auto &f : pl->fr) {
+        drop_kspace_potential(pl, f);
         k_potential<<<nblk(pl->npts, 256), 256, 0, st>>>(f.V, c, alpha0_map, alpha0_db, y, f.omega, f.k0,
                                                            pl->damping, pl->npts);
         f.have_V = true;
@@ -436,19 +599,25 @@ tbs_status tbs_set_medium(tbs_plan *pl, const float *c, const float *rho, const 
 tbs_status tbs_set_medium_host(tbs_plan *pl, const float *c, const float *rho, const float *alpha0_map,
                                double alpha0_db, double y, double beta, double rho0, void *stream) {
     if (!pl || !c) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
-    // stage through W1 (>= 2 n complex = 4 n floats): c at [0, n), alpha0 map at [n, 2n)
-    float *dc = (float *)pl->W1;
+    // stage through W1 of slot 0 (>= 2 n complex = 4 n floats): c at [0, n), alpha0 map at [n, 2n)
+    float *dc = (float *)pl->slot[0].W1;
     float *da = alpha0_map ? dc + pl->npts : nullptr;
     CU(pl, cudaMemcpyAsync(dc, c, sizeof(float) * pl->npts, cudaMemcpyHostToDevice, st));
     if (alpha0_map) CU(pl, cudaMemcpyAsync(da, alpha0_map, sizeof(float) * pl->npts, cudaMemcpyHostToDevice, st));
-    return tbs_set_medium(pl, dc, rho ? dc : nullptr, da, alpha0_db, y, beta, rho0, stream);
+    (void)rho;  // accepted for symmetry with tbs_set_medium, where it is not read either
+    return tbs_set_medium(pl, dc, nullptr, da, alpha0_db, y, beta, rho0, stream);
 }
 
 tbs_status tbs_set_potential(tbs_plan *pl, int ifreq, const float *V, void *stream) {
     if (!pl || !V || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
     Freq &f = pl->fr[ifreq];
+    drop_kspace_potential(pl, f);
     k_scale_complex<<<nblk(pl->npts, 256), 256, 0, st>>>(f.V, (const float2 *)V, 1.0 / (f.k0 * f.k0), pl->npts);
     CU(pl, cudaGetLastError());
     CU(pl, cudaStreamSynchronize(st));
@@ -464,32 +633,34 @@ tbs_status tbs_set_source(tbs_plan *pl, int n_src, const double *pos_m, const fl
             if (!(g >= 0.0) || g > (double)(pl->n[a] - 1))
                 return fail(pl, TBS_ERR_INVALID_ARG, "source %d lies outside the grid", j);
         }
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
-    double *dpos = nullptr;
-    float2 *damp = nullptr;
     const size_t nf = pl->fr.size();
-    CU(pl, cudaMalloc((void **)&dpos, sizeof(double) * n_src * pl->ndim));
-    cudaError_t e = cudaMalloc((void **)&damp, sizeof(float2) * n_src * nf);
-    if (e != cudaSuccess) { cudaFree(dpos); return fail(pl, TBS_ERR_ALLOC, "cudaMalloc(amp)"); }
-    cudaMemcpyAsync(dpos, pos_m, sizeof(double) * n_src * pl->ndim, cudaMemcpyHostToDevice, st);
-    cudaMemcpyAsync(damp, amp, sizeof(float2) * n_src * nf, cudaMemcpyHostToDevice, st);
+    const size_t pos_bytes = align_up(sizeof(double) * n_src * pl->ndim);
+    const size_t amp_bytes = sizeof(float2) * n_src * nf;
+    tbs_status ss = ensure_stage(pl, pos_bytes + amp_bytes);
+    if (ss != TBS_OK) return ss;
+    double *dpos = (double *)pl->stage;
+    float2 *damp = (float2 *)((char *)pl->stage + pos_bytes);
+    CU(pl, cudaMemcpyAsync(dpos, pos_m, sizeof(double) * n_src * pl->ndim, cudaMemcpyHostToDevice, st));
+    CU(pl, cudaMemcpyAsync(damp, amp, amp_bytes, cudaMemcpyHostToDevice, st));
     for (size_t i = 0; i < nf; ++i) {
         Freq &f = pl->fr[i];
-        cudaMemsetAsync(f.S, 0, sizeof(float2) * pl->npts, st);
+        CU(pl, cudaMemsetAsync(f.S, 0, sizeof(float2) * pl->npts, st));
         k_deposit<<<nblk((long long)n_src << pl->ndim, 128), 128, 0, st>>>(f.S, dpos, damp + i * n_src, n_src,
                                                                             pl->ndim, pl->n[0], pl->n[1], pl->n[2], pl->dx);
         f.have_S = true;
     }
-    e = cudaStreamSynchronize(st);
-    cudaFree(dpos);
-    cudaFree(damp);
-    CU(pl, e);
     CU(pl, cudaGetLastError());
+    CU(pl, cudaStreamSynchronize(st));   // the host arrays may be reused by the caller; the staging by the next call
     return TBS_OK;
 }
 
 tbs_status tbs_set_source_field(tbs_plan *pl, int ifreq, const float *S, void *stream) {
     if (!pl || !S || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
     cudaStream_t st = (cudaStream_t)stream;
     Freq &f = pl->fr[ifreq];
     CU(pl, cudaMemcpyAsync(f.S, S, sizeof(float2) * pl->npts, cudaMemcpyDeviceToDevice, st));
@@ -504,6 +675,7 @@ tbs_status tbs_get_potential(tbs_plan *pl, int ifreq, float *out, void *stream) 
     if (!f.have_V) return fail(pl, TBS_ERR_NOT_READY, "medium not set");
     cudaStream_t st = (cudaStream_t)stream;
     k_scale_complex<<<nblk(pl->npts, 256), 256, 0, st>>>((float2 *)out, f.V, f.k0 * f.k0, pl->npts);
+    CU(pl, cudaGetLastError());
     CU(pl, cudaStreamSynchronize(st));
     return TBS_OK;
 }

@@ -98,7 +98,24 @@ class Plan:
 
     # ------------------------------------------------------------------ C ABI, one method per call
     def workspace_bytes(self):
+        """tbs_plan_workspace_bytes: size of the workspace the plan needs (known before anything is allocated)."""
         return int(self._L.tbs_plan_workspace_bytes(self._h))
+
+    def set_workspace(self, buf):
+        """tbs_plan_set_workspace: run in a caller-owned CUDA tensor (any dtype, contiguous, >= workspace_bytes()).
+        The plan keeps a reference so the memory outlives it."""
+        if not (isinstance(buf, torch.Tensor) and buf.is_cuda and buf.is_contiguous()):
+            raise ValueError("workspace: expected a contiguous CUDA tensor")
+        self._check(self._L.tbs_plan_set_workspace(self._h, ctypes.c_void_p(buf.data_ptr()),
+                                                   buf.numel() * buf.element_size()))
+        self._ws = buf
+
+    def device_bytes(self):
+        return int(self._L.tbs_plan_device_bytes(self._h))
+
+    def set_concurrency(self, members):
+        """tbs_set_concurrency: members of a frequency batch solved at once (1 or 2)."""
+        self._check(self._L.tbs_set_concurrency(self._h, int(members)))
 
     def set_scheme(self, scheme):
         """tbs_set_scheme: "born" (traditional series, default) or "cbs" (convergent Born series)."""
@@ -255,6 +272,5 @@ def solve_harmonics(plans, max_terms, tol, ref_row, surface_pressure_pa):
 
 
 def grid_harmonic_frequency(m, c0, n, dx):
-    """The m-th multiple of the fundamental frequency a periodic n-point grid supports, c0/(n dx)
-    (f = 55 v_f/(4096 dx) = 1 007 080 Hz)."""
-    return m * c0 / (n * dx)
+    """tbs_grid_harmonic_frequency: the m-th frequency a periodic n-point grid carries exactly."""
+    return float(_lib.load().tbs_grid_harmonic_frequency(int(m), float(c0), int(n), float(dx)))

@@ -137,3 +137,89 @@ def test_timing_reduction_over_gloo_world_size_2(tmp_path):
         out, err = p.communicate(timeout=120)
         assert p.returncode == 0, err
         assert "ok" in out
+
+
+def test_grid_harmonic_frequency_is_the_papers_number(golden):
+    """tbs_grid_harmonic_frequency needs no device: f = 55 v_f/(4096 dx) = 1 007 080 Hz."""
+    L, _ = _lib()
+    f = L.tbs_grid_harmonic_frequency(int(golden["f_multiple"]), golden["v_f"], 4096, golden["dx_m"])
+    assert abs(f - golden["f_hz"]) < 1.0
+    assert L.tbs_grid_harmonic_frequency(0, 1500.0, 4096, 2e-5) == 0.0
+
+
+def test_workspace_calls_reject_null_arguments():
+    L, _ = _lib()
+    assert L.tbs_plan_set_workspace(None, None, 0) == -1
+    assert L.tbs_plan_device_bytes(None) == 0
+    assert L.tbs_set_concurrency(None, 2) == -1
+
+
+_SHARD_WORKER = r"""
+import ctypes, os, sys, time
+sys.path.insert(0, {root!r})
+import numpy as np
+import torch, torch.distributed as dist
+import tbs_workloads as W
+from paper_2507_13754_b200 import _lib
+from paper_2507_13754_b200.parallel import reduce_timing, shard_frequencies
+rank = int(os.environ["RANK"]); world = int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+w = W.cfg5(N=32, nfreq=16)
+mine = shard_frequencies(len(w.freqs), rank, world)
+freqs = [w.freqs[i] for i in mine]
+amp = np.ascontiguousarray(w.src_amp[mine])
+assert amp.shape == (len(mine), w.src_pos.shape[0])
+# one independent plan per rank over its own block of frequencies: the arguments pass the ABI's validation
+# (TBS_OK on a GPU box, TBS_ERR_CUDA here -- never INVALID_ARG / UNSUPPORTED_SIZE); there is no CPU fallback
+L = _lib.load()
+h = ctypes.c_void_p()
+n = (ctypes.c_int32 * 3)(*w.shape[::-1])
+ff = (ctypes.c_double * len(freqs))(*freqs)
+t0 = time.perf_counter()
+st = L.tbs_plan_create(ctypes.byref(h), 3, n, w.dx, len(freqs), ff, w.c0, w.damping)
+dt = time.perf_counter() - t0
+assert st in (0, -4), st
+if st == 0:
+    assert L.tbs_plan_workspace_bytes(h) >= 8 * 32 ** 3 * (3 * len(freqs) + 2 * 6)
+    L.tbs_plan_destroy(h)
+times, counts = reduce_timing(dist, "cpu", [dt, float(rank)], [len(mine), sum(mine)])
+assert counts == [16.0, float(sum(range(16)))], counts       # every frequency owned exactly once
+assert times[1] == float(world - 1) and times[0] >= dt
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank, mine)
+"""
+
+
+def test_frequency_shard_path_end_to_end_over_gloo_world_size_2(tmp_path):
+    """NEXT-4 host logic: shard the 16-frequency batch, one independent plan per rank, reduce."""
+    _lib()
+    script = tmp_path / "shard_worker.py"
+    script.write_text(_SHARD_WORKER.format(root=ROOT))
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT="29573")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        out, err = p.communicate(timeout=300)
+        assert p.returncode == 0, err
+        outs.append(out)
+    assert "ok 0 [0, 1, 2, 3, 4, 5, 6, 7]" in outs[0] and "ok 1 [8, 9, 10, 11, 12, 13, 14, 15]" in outs[1]
+
+
+def test_bench_spawns_its_own_ranks_for_gpus_n(monkeypatch):
+    """bench.py --gpus N outside torchrun re-launches itself under torch.distributed.run with N ranks."""
+    import importlib
+    bench = importlib.import_module("bench")
+    seen = {}
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: seen.setdefault("cmd", cmd) and 0)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4", "--steps", "2"])
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    with pytest.raises(SystemExit) as e:
+        bench.main()
+    assert e.value.code == 0
+    cmd = seen["cmd"]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=4" in cmd and "--master-addr" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[-4:] == ["--gpus", "4", "--steps", "2"]
