@@ -41,6 +41,8 @@ UNIT = "grid-point-terms/s"
 # algorithmic bytes per grid point per launch (fused-across-term figures)
 ALG_BYTES = {2: {"k_row": 56.0, "k_conv": 32.0},
              3: {"k_row": 56.0, "k_col_fwd_y": 48.0, "k_conv_z": 64.0, "k_col_inv_y": 48.0}}
+# the unpadded periodic form (2-D, the paper's own boundary): W is N wide -- 8 r + 8 w (W) + 16 (p) + 8 (V); 8 r + 8 w
+ALG_BYTES_PERIODIC = {"k_row": 40.0, "k_conv": 16.0}
 FP32_LANES = 148 * 128      # FP32 results per clock (a packed f32x2 instruction counts as 2, same pipe)
 NCU_COUNTS = os.path.join(ROOT, "profiles", "r02_ncu_counts.json")
 CSRC = os.path.join(ROOT, "paper_2507_13754_b200", "csrc")
@@ -68,11 +70,20 @@ def ncu_counts(workload_key):
     return d.get("workloads", {}).get(workload_key, {}), d.get("captured_by")
 
 
+def cfg3_batch(nf):
+    """cfg3 (2-D 2048^2) as a broadband batch: nf frequencies 1.4 ... 2.0 MHz on the same grid and medium."""
+    w = W.cfg3()
+    w.freqs = [1.4e6 + 0.6e6 * i / max(nf - 1, 1) for i in range(nf)]
+    w.src_amp = np.repeat(w.src_amp, nf, axis=0)
+    w.name += "_f%d" % nf
+    return w
+
+
 def make_workload(name):
     table = {
         "cfg1": lambda: W.cfg1(), "cfg2": lambda: W.cfg2(), "cfg3": lambda: W.cfg3(), "cfg4": lambda: W.cfg4(),
-        "cfg5": lambda: W.cfg5(), "cfg5_batch16": lambda: W.cfg5(nfreq=16),
-        "cfg3_small": lambda: W.cfg3(N=256), "cfg5_small_batch16": lambda: W.cfg5(N=64, nfreq=16),
+        "cfg5": lambda: W.cfg5(), "cfg5_batch16": lambda: W.cfg5(nfreq=16), "cfg3_batch4": lambda: cfg3_batch(4),
+        "cfg3_small": lambda: W.cfg3(N=256), "cfg5_small": lambda: W.cfg5(N=64), "cfg5_small_batch16": lambda: W.cfg5(N=64, nfreq=16),
         "paper_e1": lambda: W.paper_e1(),          # the paper's own homogeneous case, paper-faithful options
         "paper_e1_small": lambda: W.paper_e1(N=512),
     }
@@ -186,6 +197,10 @@ def run_reference(args, w):
         "gpu_launches": 0}))
 
 
+def alg_bytes(w):
+    return ALG_BYTES_PERIODIC if w.notes.get("boundary") == "periodic" and w.ndim == 2 else ALG_BYTES[w.ndim]
+
+
 def kernel_report(plan, w, workload_key, peak, sm_mhz):
     """Per-kernel device time of one term (tbs_profile_term: each kernel launched back to back between two CUDA
     events on the launching stream) and the roofline of each: algorithmic bytes / duration vs the HBM peak."""
@@ -193,8 +208,9 @@ def kernel_report(plan, w, workload_key, peak, sm_mhz):
     counts, captured_by = ncu_counts(workload_key)
     clock_hz = (sm_mhz or 1965.0) * 1e6
     kernels = []
-    for name, ms in zip(ALG_BYTES[w.ndim].keys(), kms):
-        b = ALG_BYTES[w.ndim][name] * w.n_points
+    alg = alg_bytes(w)
+    for name, ms in zip(alg.keys(), kms):
+        b = alg[name] * w.n_points
         k = {"kernel": name, "ms": float(ms), "alg_bytes": b, "achieved_gbs": b / (ms * 1e-3) / 1e9,
              "frac": b / (ms * 1e-3) / 1e9 / peak}
         c = counts.get(name)
@@ -224,6 +240,8 @@ def measure(args, w, workload_key, steps, warmup, with_e2e, dist, rank, world, l
     nf = len(w.freqs)
 
     plan = Plan(w.shape, w.dx, w.freqs, w.c0, w.damping)
+    if args.launch_overlap is not None:
+        plan.set_launch_overlap(args.launch_overlap)
     if args.concurrency is not None and nf > 1:
         plan.set_concurrency(args.concurrency)
     # torch owns the device memory the solve runs in (north_star: "PyTorch is used only for device memory and streams")
@@ -305,7 +323,7 @@ def measure(args, w, workload_key, steps, warmup, with_e2e, dist, rank, world, l
     kernels, captured_by = kernel_report(plan, w, workload_key, peak, clocks.get("sm_mhz"))
     dom = max(kernels, key=lambda k: k["ms"])
     term_ms = loop_ms / max(local_terms, 1)
-    term_bytes = sum(ALG_BYTES[w.ndim].values()) * w.n_points
+    term_bytes = sum(alg_bytes(w).values()) * w.n_points
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
                 "unit": "GB/s", "frac": dom["frac"], "traffic": dom.get("dram_traffic_ncu"),
                 "peak_source": peak_src}
@@ -361,6 +379,7 @@ def main():
     ap.add_argument("--ref-terms", type=int, default=2, help="Born terms per step of the oracle arm")
     ap.add_argument("--cpu-baseline-terms", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--launch-overlap", type=int, default=None, help="0: plain stream order between the term kernels")
     ap.add_argument("--concurrency", type=int, default=None, help="members of a frequency batch in flight (1 or 2)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "frequencies"],
                     help="N>1: independent replicas (weak) or shard the frequency batch (strong)")

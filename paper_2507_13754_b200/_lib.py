@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libtbs.so")
 # every symbol include/tbs.h declares
 SYMBOLS = [
     "tbs_version", "tbs_plan_create", "tbs_plan_destroy", "tbs_plan_workspace_bytes", "tbs_plan_set_workspace",
-    "tbs_plan_device_bytes", "tbs_grid_harmonic_frequency", "tbs_set_concurrency", "tbs_last_error",
+    "tbs_plan_device_bytes", "tbs_grid_harmonic_frequency", "tbs_set_concurrency", "tbs_set_launch_overlap", "tbs_last_error",
     "tbs_set_abl", "tbs_set_scheme", "tbs_set_boundary", "tbs_set_criterion", "tbs_set_kspace_absorption", "tbs_set_medium", "tbs_set_medium_host", "tbs_set_potential", "tbs_set_source",
     "tbs_set_source_field", "tbs_solve", "tbs_solve_host", "tbs_solve_second_harmonic", "tbs_solve_harmonics",
     "tbs_apply_green", "tbs_get_potential", "tbs_get_source", "tbs_green_spectrum",
@@ -50,6 +50,7 @@ def load() -> ctypes.CDLL:
     L.tbs_grid_harmonic_frequency.argtypes = [i32, dbl, i32, dbl]
     L.tbs_grid_harmonic_frequency.restype = dbl
     L.tbs_set_concurrency.argtypes = [vp, i32]
+    L.tbs_set_launch_overlap.argtypes = [vp, i32]
     L.tbs_last_error.argtypes = [vp]
     L.tbs_last_error.restype = ctypes.c_char_p
     L.tbs_set_abl.argtypes = [vp, i32, dbl]

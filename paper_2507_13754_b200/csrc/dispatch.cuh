@@ -40,28 +40,34 @@ template <> struct ConvCfg<4096> { static constexpr int T = 2, MINB = 1; };
 //                  general variant when a.ucbs or a.crit_row >= 0 asks for it)
 //   launch_conv_n: k_conv (general variant for the k-space potential / masked periodic tables)
 //   launch_col_n : k_col, mode = MODE_FWD or MODE_INV (3-D y passes; lengths <= 512)
-// `sm_limit` > 0 caps the persistent grid to that many SMs' worth of CTAs (frequency batch: members share the GPU).
-template <int N> cudaError_t launch_row_n(bool first, const RowArgs &a, cudaStream_t st, bool set_attr, int sm_limit);
+// LaunchOpt: sm_limit > 0 caps the persistent grid to that many SMs' worth of CTAs (frequency batch: members share
+// the GPU); overlap: programmatic dependent launch -- the kernel may be scheduled while its predecessor in the
+// stream drains (every kernel waits with griddepcontrol.wait before it touches memory).
+struct LaunchOpt {
+    int sm_limit = 0;
+    bool overlap = false;
+};
+template <int N> cudaError_t launch_row_n(bool first, const RowArgs &a, cudaStream_t st, bool set_attr, LaunchOpt opt);
 template <int N> cudaError_t launch_conv_n(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st,
-                                           bool set_attr, int sm_limit);
+                                           bool set_attr, LaunchOpt opt);
 template <int N> cudaError_t launch_col_n(int mode, const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr,
-                                          int sm_limit);
+                                          LaunchOpt opt);
 
 #define TBS_FOR_EACH_N(X) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096)
 
 // Every length is instantiated explicitly in its own translation unit (inst.cu): keep the switches below from
 // instantiating all of them wherever the definitions of dispatch_impl.cuh are visible.
 #define X(n)                                                                                                          \
-    extern template cudaError_t launch_row_n<n>(bool, const RowArgs &, cudaStream_t, bool, int);                       \
-    extern template cudaError_t launch_conv_n<n>(const ColArgs &, const CUtensorMap *, int, cudaStream_t, bool, int); \
-    extern template cudaError_t launch_col_n<n>(int, const ColArgs &, int, cudaStream_t, bool, int);
+    extern template cudaError_t launch_row_n<n>(bool, const RowArgs &, cudaStream_t, bool, LaunchOpt);                       \
+    extern template cudaError_t launch_conv_n<n>(const ColArgs &, const CUtensorMap *, int, cudaStream_t, bool, LaunchOpt); \
+    extern template cudaError_t launch_col_n<n>(int, const ColArgs &, int, cudaStream_t, bool, LaunchOpt);
 TBS_FOR_EACH_N(X)
 #undef X
 
 static inline cudaError_t launch_row(int N, bool first, const RowArgs &a, cudaStream_t st, bool set_attr = false,
-                                     int sm_limit = 0) {
+                                     LaunchOpt opt = LaunchOpt()) {
     switch (N) {
-#define X(n) case n: return launch_row_n<n>(first, a, st, set_attr, sm_limit);
+#define X(n) case n: return launch_row_n<n>(first, a, st, set_attr, opt);
         TBS_FOR_EACH_N(X)
 #undef X
         default: break;
@@ -70,9 +76,9 @@ static inline cudaError_t launch_row(int N, bool first, const RowArgs &a, cudaSt
 }
 
 static inline cudaError_t launch_conv(int N, const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st,
-                                      bool set_attr = false, int sm_limit = 0) {
+                                      bool set_attr = false, LaunchOpt opt = LaunchOpt()) {
     switch (N) {
-#define X(n) case n: return launch_conv_n<n>(a, tmap, n_outer, st, set_attr, sm_limit);
+#define X(n) case n: return launch_conv_n<n>(a, tmap, n_outer, st, set_attr, opt);
         TBS_FOR_EACH_N(X)
 #undef X
         default: break;
@@ -81,13 +87,13 @@ static inline cudaError_t launch_conv(int N, const ColArgs &a, const CUtensorMap
 }
 
 static inline cudaError_t launch_col(int N, int mode, const ColArgs &a, int n_outer, cudaStream_t st,
-                                     bool set_attr = false, int sm_limit = 0) {
+                                     bool set_attr = false, LaunchOpt opt = LaunchOpt()) {
     switch (N) {
-        case 32:   return launch_col_n<32>(mode, a, n_outer, st, set_attr, sm_limit);
-        case 64:   return launch_col_n<64>(mode, a, n_outer, st, set_attr, sm_limit);
-        case 128:  return launch_col_n<128>(mode, a, n_outer, st, set_attr, sm_limit);
-        case 256:  return launch_col_n<256>(mode, a, n_outer, st, set_attr, sm_limit);
-        case 512:  return launch_col_n<512>(mode, a, n_outer, st, set_attr, sm_limit);
+        case 32:   return launch_col_n<32>(mode, a, n_outer, st, set_attr, opt);
+        case 64:   return launch_col_n<64>(mode, a, n_outer, st, set_attr, opt);
+        case 128:  return launch_col_n<128>(mode, a, n_outer, st, set_attr, opt);
+        case 256:  return launch_col_n<256>(mode, a, n_outer, st, set_attr, opt);
+        case 512:  return launch_col_n<512>(mode, a, n_outer, st, set_attr, opt);
         default: break;
     }
     return cudaErrorInvalidValue;

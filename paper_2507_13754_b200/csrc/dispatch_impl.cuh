@@ -21,8 +21,26 @@ static inline Resident resident_ctas(const void *kern, int threads, size_t smem)
     return r;
 }
 
+// One launch; overlap = programmatic stream serialization (the kernel's CTAs may become resident while the
+// previous kernel of the stream drains; griddepcontrol.wait in the kernel orders the memory accesses).
+template <class... KArgs, class... Args>
+static cudaError_t launch_k(void (*kern)(KArgs...), unsigned grid, int threads, size_t smem, cudaStream_t st, bool overlap,
+                            Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = overlap ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 template <int N, int MODE>
-static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr, int sm_limit) {
+static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr, LaunchOpt opt) {
     using C = ColCfg<N>;
     constexpr size_t smem = (size_t)N * C::T * sizeof(float2) * (MODE == MODE_INV ? 2 : 3);
     auto kern = k_col<N, C::T, C::NT, MODE>;
@@ -35,18 +53,17 @@ static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, 
     ColArgs b = a;
     b.n_outer = n_outer;
     const long long total = (long long)n_outer * (a.inner_len / C::T);
-    const long long cap = res.cap(sm_limit);
-    kern<<<(unsigned)(total < cap ? total : cap), C::NT, smem, st>>>(b);
-    return cudaGetLastError();
+    const long long cap = res.cap(opt.sm_limit);
+    return launch_k(kern, (unsigned)(total < cap ? total : cap), C::NT, smem, st, opt.overlap, b);
 }
 
-template <int N, bool KABS>
+template <int N, bool KABS, bool PER = false>
 static cudaError_t launch_conv_tt(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr,
-                                  int sm_limit) {
+                                  LaunchOpt opt) {
     constexpr int T = ConvCfg<N>::T;
-    constexpr int NT = T * tpl_of(N);
-    constexpr size_t smem = (size_t)conv_smem_bytes(N, T);
-    auto kern = k_conv<N, T, ConvCfg<N>::MINB, KABS>;
+    constexpr int NT = (PER ? T / 2 : T) * tpl_of(N);
+    constexpr size_t smem = PER ? (size_t)conv_smem_bytes_per(N, T) : (size_t)conv_smem_bytes(N, T);
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB, KABS, PER>;
     static Resident res;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -56,13 +73,12 @@ static cudaError_t launch_conv_tt(const ColArgs &a, const CUtensorMap *tmap, int
     ColArgs b = a;
     b.n_outer = n_outer;
     const long long total = (long long)n_outer * (a.inner_len / T);
-    const long long cap = res.cap(sm_limit);
-    kern<<<(unsigned)(total < cap ? total : cap), NT, smem, st>>>(b, *tmap);
-    return cudaGetLastError();
+    const long long cap = res.cap(opt.sm_limit);
+    return launch_k(kern, (unsigned)(total < cap ? total : cap), NT, smem, st, opt.overlap, b, *tmap);
 }
 
-template <int N, bool FIRST, bool GEN>
-static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr, int sm_limit) {
+template <int N, bool FIRST, bool GEN, bool PER = false>
+static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr, LaunchOpt opt) {
     using C = RowCfg<N>;
     constexpr int TPL = row_tpl_of(N);
     constexpr int GR = TPL >= 32 ? 1 : 32 / TPL;
@@ -70,51 +86,57 @@ static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_att
     constexpr int ROWS = C::GROUPS * GR;
     constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
                             (FIRST || !row_staged(N) ? 0 : (size_t)ROWS * N * sizeof(float4));
-    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN>;
+    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN, PER>;
     static Resident res;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) res = resident_ctas((const void *)kern, NT, smem);
         return e;
     }
-    const long long tiles = (a.rows / GR + C::GROUPS - 1) / C::GROUPS;
-    const long long cap = res.cap(sm_limit);
-    kern<<<(unsigned)(tiles < cap ? tiles : cap), NT, smem, st>>>(a);
-    return cudaGetLastError();
+    const long long tiles = (a.rows / (GR * (PER ? 2 : 1)) + C::GROUPS - 1) / C::GROUPS;
+    const long long cap = res.cap(opt.sm_limit);
+    return launch_k(kern, (unsigned)(tiles < cap ? tiles : cap), NT, smem, st, opt.overlap, a);
 }
 
 template <int N>
-cudaError_t launch_row_n(bool first, const RowArgs &a, cudaStream_t st, bool set_attr, int sm_limit) {
+cudaError_t launch_row_n(bool first, const RowArgs &a, cudaStream_t st, bool set_attr, LaunchOpt opt) {
     if (set_attr) {
-        cudaError_t e = launch_row_tt<N, true, false>(a, st, true, 0);
-        if (e == cudaSuccess) e = launch_row_tt<N, false, false>(a, st, true, 0);
-        if (e == cudaSuccess) e = launch_row_tt<N, false, true>(a, st, true, 0);
+        cudaError_t e = launch_row_tt<N, true, false>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, false, false>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, false, true>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, true, false, true>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, false, true, true>(a, st, true, LaunchOpt());
         return e;
     }
-    if (first) return launch_row_tt<N, true, false>(a, st, false, sm_limit);
-    return (a.ucbs || a.crit_row >= 0) ? launch_row_tt<N, false, true>(a, st, false, sm_limit)
-                                        : launch_row_tt<N, false, false>(a, st, false, sm_limit);
+    if (a.per) return first ? launch_row_tt<N, true, false, true>(a, st, false, opt)
+                            : launch_row_tt<N, false, true, true>(a, st, false, opt);
+    if (first) return launch_row_tt<N, true, false>(a, st, false, opt);
+    return (a.ucbs || a.crit_row >= 0) ? launch_row_tt<N, false, true>(a, st, false, opt)
+                                        : launch_row_tt<N, false, false>(a, st, false, opt);
 }
 
 template <int N>
 cudaError_t launch_conv_n(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr,
-                          int sm_limit) {
+                          LaunchOpt opt) {
     if (set_attr) {
-        cudaError_t e = launch_conv_tt<N, false>(a, tmap, n_outer, st, true, 0);
-        return e != cudaSuccess ? e : launch_conv_tt<N, true>(a, tmap, n_outer, st, true, 0);
+        cudaError_t e = launch_conv_tt<N, false>(a, tmap, n_outer, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_conv_tt<N, true>(a, tmap, n_outer, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_conv_tt<N, true, true>(a, tmap, n_outer, st, true, LaunchOpt());
+        return e;
     }
-    return a.kabs.nu > 0.f || a.masked ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false, sm_limit)
-                                       : launch_conv_tt<N, false>(a, tmap, n_outer, st, false, sm_limit);
+    if (a.per) return launch_conv_tt<N, true, true>(a, tmap, n_outer, st, false, opt);
+    return a.kabs.nu > 0.f || a.masked ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false, opt)
+                                       : launch_conv_tt<N, false>(a, tmap, n_outer, st, false, opt);
 }
 
 template <int N>
-cudaError_t launch_col_n(int mode, const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr, int sm_limit) {
+cudaError_t launch_col_n(int mode, const ColArgs &a, int n_outer, cudaStream_t st, bool set_attr, LaunchOpt opt) {
     if (set_attr) {
-        cudaError_t e = launch_col_t<N, MODE_FWD>(a, n_outer, st, true, 0);
-        return e != cudaSuccess ? e : launch_col_t<N, MODE_INV>(a, n_outer, st, true, 0);
+        cudaError_t e = launch_col_t<N, MODE_FWD>(a, n_outer, st, true, LaunchOpt());
+        return e != cudaSuccess ? e : launch_col_t<N, MODE_INV>(a, n_outer, st, true, LaunchOpt());
     }
-    return mode == MODE_FWD ? launch_col_t<N, MODE_FWD>(a, n_outer, st, false, sm_limit)
-                            : launch_col_t<N, MODE_INV>(a, n_outer, st, false, sm_limit);
+    return mode == MODE_FWD ? launch_col_t<N, MODE_FWD>(a, n_outer, st, false, opt)
+                            : launch_col_t<N, MODE_INV>(a, n_outer, st, false, opt);
 }
 
 }  // namespace tbs

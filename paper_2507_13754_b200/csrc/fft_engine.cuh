@@ -72,6 +72,21 @@ __device__ __forceinline__ void cp_async16(void *dst, const void *src) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+// Programmatic dependent launch: let the next kernel of the stream be scheduled while this one drains / wait
+// for the previous kernel of the stream to complete and its writes to be visible (no-ops without the attribute).
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Streaming accesses of the fields (read or written once per term): keep them out of L1, which holds the tables.
+__device__ __forceinline__ float2 ld_stream(const float2 *p) {
+    float2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ld_stream_nc(const float2 *p) {
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ---- radix plan ------------------------------------------------------------------------------
@@ -209,6 +224,8 @@ __host__ __device__ constexpr bool conv_p2_in_smem(int N, int T) {
 __host__ __device__ constexpr int conv_smem_bytes(int N, int T) {
     return conv_stage_offset(N, T) + N * T * 8 + (conv_p2_in_smem(N, T) ? conv_lutc_entries(N) * 8 + N * 8 : 0);
 }
+// the periodic form of k_conv (T/2 line slots per tile, no table copies)
+__host__ __device__ constexpr int conv_smem_bytes_per(int N, int T) { return conv_stage_offset(N, T / 2) + N * T * 8; }
 __host__ __device__ constexpr int tpl_of(int N) { return N / 16 >= 4 ? N / 16 : 4; }
 // k_conv: first/last-stage items per line >= threads of two lines (N = 512, 1024, 2048): the fused last/first
 // stage runs by line pairs with 16-byte accesses to the tile buffer.

@@ -234,6 +234,39 @@ __device__ __forceinline__ void pfirst_fwd_tw(const float2 (&x)[R1], int line, i
     for (int i = 0; i < R1; ++i) sts_p2(sm + Lay::addr(line, t + brev(i, R1) * S1), v[i]);
 }
 
+// Periodic (unpadded) form: the two lanes of a value are two independent lines A and B (adjacent rows in k_row,
+// adjacent columns in k_conv) that share every twiddle; xa, xb are their inputs at position t + j*S1.  The
+// table passed as wre/wim holds w_N^(k t) in both lanes.
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void pfirst_fwd_2l(const float2 (&xa)[R1], const float2 (&xb)[R1], int line, int t, float4 *sm,
+                                              const float2 (&wre)[R1], const float2 (&wim)[R1]) {
+    constexpr int S1 = N / R1;
+    P2 v[R1];
+#pragma unroll
+    for (int j = 0; j < R1; ++j) v[j] = P2{make_float2(xa[j].x, xb[j].x), make_float2(xa[j].y, xb[j].y)};
+    pbfly<R1, -1>(v);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) v[i] = pmul2(v[i], wre[brev(i, R1)], wim[brev(i, R1)]);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) sts_p2(sm + Lay::addr(line, t + brev(i, R1) * S1), v[i]);
+}
+// Last inverse stage of the periodic form: za[j], zb[j] = IFFT_N of line A, B at position t + j*S1.
+template <int N, int R1, class Lay>
+__device__ __forceinline__ void plast_inv_2l(float2 (&za)[R1], float2 (&zb)[R1], int line, int t, const float4 *sm,
+                                             const float2 (&wre)[R1], const float2 (&wim)[R1]) {
+    constexpr int S1 = N / R1;
+    P2 v[R1];
+#pragma unroll
+    for (int k = 0; k < R1; ++k) v[k] = lds_p2(sm + Lay::addr(line, t + k * S1));
+    pbfly_dit<R1>(v, wre, wim);
+#pragma unroll
+    for (int i = 0; i < R1; ++i) {
+        const int j = brev(i, R1);
+        za[j] = make_float2(v[i].re.x, v[i].im.x);
+        zb[j] = make_float2(v[i].re.y, v[i].im.y);
+    }
+}
+
 template <int N, int R1, class Lay>
 __device__ __forceinline__ void pfirst_fwd(const float2 (&x)[R1], int line, int t, float4 *sm,
                                            const float4 *__restrict__ lutAB) {
@@ -275,7 +308,8 @@ __device__ __forceinline__ void plast_inv(float2 (&z)[R1], int line, int t, cons
 // so v ghat = ((v.re alpha - v.im) + i (v.im alpha + v.re)) / (alpha^2 + 1): six packed operations
 // and one MUFU.RCP per half; the constant 1/(e k0^2) rides on the normalisation applied by k_row.
 // p2x2: the line-axis table |p|^2/(e k0^2), interleaved over the halves, [j][block] float2 = (even, odd);
-// a_line: (|p|^2 of the other axes / k0^2 - 1) / e.
+// a_line: (|p|^2 of the other axes / k0^2 - 1) / e, per lane (equal lanes for a padded line; the two columns'
+// values in the periodic form).
 template <int N, int RL, bool TSM>
 __device__ __forceinline__ void load_p2x2(float2 (&pp)[RL], const float2 *__restrict__ p2x2, int b) {
 #pragma unroll
@@ -291,7 +325,7 @@ struct KAbs {
 // (homogeneous absorbing-dispersive medium, Eq. 24); kappa^2 = 1 + e alpha comes from the same tables.
 template <int N, int RL, class Lay, bool TSM = false, bool KABS = false>
 __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
-                                               float a_line, KAbs ka = KAbs{0.f, 0.f, 0.f, 0.f}) {
+                                               float2 a_line, KAbs ka = KAbs{0.f, 0.f, 0.f, 0.f}) {
     const int base = b * RL;
     float2 pp[RL];
     load_p2x2<N, RL, TSM>(pp, p2x2, b);
@@ -308,7 +342,7 @@ __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, cons
 #pragma unroll
         for (int i = 0; i < RL; ++i) {
             const int k = brev(i, RL);
-            const float2 al = __fadd2_rn(pp[k], f2(a_line));
+            const float2 al = __fadd2_rn(pp[k], a_line);
             const float2 d = __ffma2_rn(al, al, f2(1.0f));
             const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
             const P2 t = P2{__ffma2_rn(v[i].re, al, neg2(v[i].im)), __ffma2_rn(v[i].im, al, v[i].re)};
@@ -333,7 +367,7 @@ __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, cons
 #pragma unroll
         for (int i = 0; i < RL; ++i) {
             const int k = brev(i, RL);
-            const float2 al = __fadd2_rn(pp[k], f2(a_line));
+            const float2 al = __fadd2_rn(pp[k], a_line);
             const float2 d = __ffma2_rn(al, al, f2(1.0f));
             const float2 r = make_float2(rcp_fast(d.x), rcp_fast(d.y));
             P2 w = P2{__fmul2_rn(__ffma2_rn(v[i].re, al, neg2(v[i].im)), r), __fmul2_rn(__ffma2_rn(v[i].im, al, v[i].re), r)};

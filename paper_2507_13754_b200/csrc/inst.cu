@@ -7,9 +7,9 @@
 #endif
 
 namespace tbs {
-template cudaError_t launch_row_n<TBS_N>(bool, const RowArgs &, cudaStream_t, bool, int);
-template cudaError_t launch_conv_n<TBS_N>(const ColArgs &, const CUtensorMap *, int, cudaStream_t, bool, int);
+template cudaError_t launch_row_n<TBS_N>(bool, const RowArgs &, cudaStream_t, bool, LaunchOpt);
+template cudaError_t launch_conv_n<TBS_N>(const ColArgs &, const CUtensorMap *, int, cudaStream_t, bool, LaunchOpt);
 #if TBS_N <= 512
-template cudaError_t launch_col_n<TBS_N>(int, const ColArgs &, int, cudaStream_t, bool, int);
+template cudaError_t launch_col_n<TBS_N>(int, const ColArgs &, int, cudaStream_t, bool, LaunchOpt);
 #endif
 }  // namespace tbs

@@ -56,6 +56,7 @@ struct ColArgs {
     float inv_e;            // k0^2/eps = 1/damping
     KAbs kabs;              // k-space multiplier potential of Eq. 24 (k_conv<..., KABS = true> only)
     int masked;             // periodic boundary: axis tables mask the odd padded frequencies (general k_conv)
+    int per;                // periodic boundary, unpadded form (k_conv<..., PER = true>; 2-D)
     Luts lut;
     const Ctl *ctl;
 };
@@ -77,6 +78,8 @@ __global__ void __launch_bounds__(NT) k_col(ColArgs a) {
     using Lay = ColLay<N, T, RL>;
     extern __shared__ __align__(1024) float2 sm[];
     float2 *stg = sm + 2 * HALF;  // [N][T] staged input tile (FWD)
+    griddep_launch();
+    griddep_wait();
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
@@ -188,6 +191,7 @@ struct RowArgs {
     float2 *ucbs;         // CBS scheme: [rows][N] current term u_n (read and replaced); nullptr for TBS
     float inv_e;          // CBS: k0^2/eps
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
+    int per;              // periodic boundary, unpadded form (k_row<..., PER = true>): W is [rows][N]
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
     Ctl *ctl;
@@ -215,7 +219,10 @@ struct RowArgs {
 // Persistent and group-independent: group G of CTA B walks row tiles (B*GROUPS + G) + i*gridDim.x*
 // GROUPS; the W rows of its next tile arrive by one bulk copy (completion on the group's mbarrier)
 // in a staging buffer while the current tile computes.
-template <int N, int GROUPS, int MINB, bool FIRST, bool GEN>
+// PER = true: the periodic (unpadded) form (Eq. 19, Alg. 1 l.36-38): one length-N transform per grid
+// row, W is [rows][N], and the two lanes of every packed value are two adjacent grid rows (a line slot = rows
+// 2s, 2s + 1); first/last-stage table with w_N^(k t) in both lanes, no padding twist, no crop.
+template <int N, int GROUPS, int MINB, bool FIRST, bool GEN, bool PER = false>
 __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) : 32), MINB) k_row(RowArgs a) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
@@ -231,7 +238,8 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
     constexpr int ROWS = GROUPS * GR;
     constexpr int NITEM = S1 / TPL;  // first/last-stage items per thread
     static_assert(S1 % TPL == 0, "items per thread");
-    constexpr bool EARLY = NITEM * R1 <= 16;  // p and V requested a barrier ahead (else per item: registers)
+    constexpr bool EARLY = !PER && NITEM * R1 <= 16;  // p and V requested a barrier ahead (else per item: registers)
+    constexpr int NR = PER ? 2 : 1;  // grid rows per line slot
     // R2 == RL: the RL x RL block a middle-stage item works in is the block of the RL contiguous-stage items of the
     // same 16 threads (item b of either stage lies in block b / RL), so the two stages only need a warp barrier.
     constexpr bool WL = warp_local_mid(R2, RL, TPL);
@@ -242,13 +250,15 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
     __shared__ float red[2][32];
     __shared__ __align__(8) uint64_t mbar[GROUPS];
     __shared__ int next_gt[GROUPS];
+    griddep_launch();
+    griddep_wait();
     if (a.ctl->done) return;
 
     const int tid = threadIdx.x;
     const int g = tid / GT, gl = tid % GT;
     const int l = g * GR + gl / TPL;  // CTA-local line
     const int lt = gl % TPL;
-    const int ngt = a.rows / GR;      // group tiles
+    const int ngt = a.rows / (GR * NR);  // group tiles
     const int gstride = gridDim.x * GROUPS;
     const int term = FIRST ? 0 : a.ctl->term;
     constexpr uint32_t TILE_BYTES = (uint32_t)GR * M * sizeof(float2);
@@ -270,19 +280,24 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
     // groups of a launch do not finish their rows at the same pace; FIRST keeps the static walk).
 #pragma unroll 1
     while (gt < ngt) {
-        const int row = gt * GR + gl / TPL;
-        float wrow = a.scale;
+        const int row = gt * GR + gl / TPL;   // line slot: grid row `row` (padded form), rows 2 row, 2 row + 1 (periodic)
+        float wrow[NR];
         float2 pold[EARLY ? NITEM : 1][R1], vpot[EARLY ? NITEM : 1][R1];
+#pragma unroll
+        for (int h = 0; h < NR; ++h) wrow[h] = a.scale;
         if (!FIRST) {
             // ---------------- inverse half: IFFT_x, crop, window, accumulate ----------------
             // pull the p and V rows of this tile towards L2 while the W rows arrive
-            for (int i = gl; i < GR * N / 16; i += GT) {
-                prefetch_l2(a.p + (long long)gt * GR * N + i * 16);
-                prefetch_l2(a.V + (long long)gt * GR * N + i * 16);
-                if (GEN && a.ucbs) prefetch_l2(a.ucbs + (long long)gt * GR * N + i * 16);
+            for (int i = gl; i < GR * NR * N / 16; i += GT) {
+                prefetch_l2(a.p + (long long)gt * GR * NR * N + i * 16);
+                prefetch_l2(a.V + (long long)gt * GR * NR * N + i * 16);
+                if (GEN && a.ucbs) prefetch_l2(a.ucbs + (long long)gt * GR * NR * N + i * 16);
             }
-            wrow *= __ldg(&a.ay[row % a.ny]);
-            if (a.az) wrow *= __ldg(&a.az[row / a.ny]);
+#pragma unroll
+            for (int h = 0; h < NR; ++h) {
+                wrow[h] *= __ldg(&a.ay[(row * NR + h) % a.ny]);
+                if (a.az) wrow[h] *= __ldg(&a.az[(row * NR + h) / a.ny]);
+            }
             if (STAGED) {
                 mbar_wait(&mbar[g], phase);
                 phase ^= 1u;
@@ -294,8 +309,16 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
                 P2 v[RL];
 #pragma unroll
                 for (int k = 0; k < RL; ++k) {
-                    const float4 f = STAGED ? stg[l * N + k * NBL + b] : wrow_g[k * NBL + b];
-                    v[k] = P2{make_float2(f.x, f.z), make_float2(f.y, f.w)};
+                    if (PER) {
+                        // rows A and B of the slot lie one behind the other (N values each)
+                        const float2 *ra = STAGED ? reinterpret_cast<const float2 *>(stg + l * N)
+                                                  : reinterpret_cast<const float2 *>(wrow_g);
+                        const float2 fa = ra[k * NBL + b], fb = ra[N + k * NBL + b];
+                        v[k] = P2{make_float2(fa.x, fb.x), make_float2(fa.y, fb.y)};
+                    } else {
+                        const float4 f = STAGED ? stg[l * N + k * NBL + b] : wrow_g[k * NBL + b];
+                        v[k] = P2{make_float2(f.x, f.z), make_float2(f.y, f.w)};
+                    }
                 }
                 pbfly<RL, +1>(v);
 #pragma unroll
@@ -328,8 +351,8 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
                     for (int j = 0; j < R1; ++j) {
                         const long long gi = (long long)row * N + lt + it * TPL + j * S1;
-                        pold[it][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
-                        vpot[it][j] = __ldg(&a.V[gi]);
+                        pold[it][j] = term > 0 ? ld_stream(&a.p[gi]) : make_float2(0.f, 0.f);
+                        vpot[it][j] = ld_stream_nc(&a.V[gi]);
                     }
             }
             if (R2 > 0) group_sync<GT>(g);
@@ -341,34 +364,49 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
         for (int it = 0; it < NITEM; ++it) {
             const int t = lt + it * TPL;
-            float2 x[R1];
+            // x[h][j]: line h of the slot (the one padded line, or the two grid rows of the periodic form) at
+            // position t + j*S1 -- first the inverse transform's output, then the input of the forward half
+            float2 x[NR][R1];
             float2 wre[R1], wim[R1];
             load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
             constexpr int pi = EARLY ? 1 : 0;
             const int ii = it * pi;  // slot of this item's p and V values
             if (!FIRST) {
+                if (PER) plast_inv_2l<N, R1, Lay>(x[0], x[NR - 1], l, t, wk, wre, wim);
+                else plast_inv_tw<N, R1, Lay>(x[0], l, t, wk, wre, wim);
+            }
+#pragma unroll
+            for (int h = 0; h < NR; ++h) {
+                const int grow = row * NR + h;  // grid row
+                if (FIRST) {
+#pragma unroll
+                    for (int j = 0; j < R1; ++j) {
+                        const float2 v = ld_stream_nc(&a.src[(long long)grow * N + t + j * S1]);
+                        x[h][j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
+                    }
+                    continue;
+                }
                 if (!EARLY) {
 #pragma unroll
                     for (int j = 0; j < R1; ++j) {
-                        const long long gi = (long long)row * N + t + j * S1;
-                        pold[0][j] = term > 0 ? a.p[gi] : make_float2(0.f, 0.f);
-                        vpot[0][j] = __ldg(&a.V[gi]);
+                        const long long gi = (long long)grow * N + t + j * S1;
+                        pold[0][j] = term > 0 ? ld_stream(&a.p[gi]) : make_float2(0.f, 0.f);
+                        vpot[0][j] = ld_stream_nc(&a.V[gi]);
                     }
                 }
-                plast_inv_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
                 // The run-time options of the general variant are tested around whole loops over the R1
                 // outputs, never inside them: the loop bodies stay branch-free and interleave.
                 float2 uv[R1];
 #pragma unroll
                 for (int j = 0; j < R1; ++j) {
-                    const float wgt = wrow * __ldg(&a.ax[t + j * S1]);
-                    uv[j] = make_float2(x[j].x * wgt, x[j].y * wgt);
+                    const float wgt = wrow[h] * __ldg(&a.ax[t + j * S1]);
+                    uv[j] = make_float2(x[h][j].x * wgt, x[h][j].y * wgt);
                 }
                 if (GEN && a.ucbs) {
                     // convergent Born series: u_{n+1} = u_n + gamma (A G(V u_n) - u_n), gamma = i V / eps
 #pragma unroll
                     for (int j = 0; j < R1; ++j) {
-                        const long long gi = (long long)row * N + t + j * S1;
+                        const long long gi = (long long)grow * N + t + j * S1;
                         const float2 gam = make_float2(-vpot[ii][j].y * a.inv_e, vpot[ii][j].x * a.inv_e);
                         const float2 uo = term > 0 ? a.ucbs[gi] : make_float2(0.f, 0.f);
                         uv[j] = cadd(uo, cmul(gam, csub(uv[j], uo)));
@@ -379,13 +417,13 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
                     for (int j = 0; j < R1; ++j) {
                         const float2 pv = cadd(pold[ii][j], uv[j]);
-                        a.p[(long long)row * N + t + j * S1] = pv;
+                        a.p[(long long)grow * N + t + j * S1] = pv;
                         uu = fmaf(uv[j].x, uv[j].x, fmaf(uv[j].y, uv[j].y, uu));
                         pp = fmaf(pv.x, pv.x, fmaf(pv.y, pv.y, pp));
                     }
-                } else if (row != a.crit_row) {
+                } else if (grow != a.crit_row) {
 #pragma unroll
-                    for (int j = 0; j < R1; ++j) a.p[(long long)row * N + t + j * S1] = cadd(pold[ii][j], uv[j]);
+                    for (int j = 0; j < R1; ++j) a.p[(long long)grow * N + t + j * S1] = cadd(pold[ii][j], uv[j]);
                 } else {
                     // Eq. 30: sum |psi_{l+1} - psi_l| and sum |psi_l| on one row; moduli through a 2^20 pre-scale
                     // (the squares stay in range for 1e-25 < |.| < 1e13)
@@ -393,23 +431,18 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
                     for (int j = 0; j < R1; ++j) {
                         const float2 po = pold[ii][j];
-                        a.p[(long long)row * N + t + j * S1] = cadd(po, uv[j]);
+                        a.p[(long long)grow * N + t + j * S1] = cadd(po, uv[j]);
                         const float ax = uv[j].x * SC, ay = uv[j].y * SC, bx = po.x * SC, by = po.y * SC;
                         uu = fmaf(sqrtf(fmaf(ax, ax, ay * ay)), ISC, uu);
                         pp = fmaf(sqrtf(fmaf(bx, bx, by * by)), ISC, pp);
                     }
                 }
 #pragma unroll
-                for (int j = 0; j < R1; ++j) x[j] = cmul(vpot[ii][j], uv[j]);
-                if (!a.do_fwd) continue;
-            } else {
-#pragma unroll
-                for (int j = 0; j < R1; ++j) {
-                    const float2 v = a.src[(long long)row * N + t + j * S1];
-                    x[j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
-                }
+                for (int j = 0; j < R1; ++j) x[h][j] = cmul(vpot[ii][j], uv[j]);
             }
-            pfirst_fwd_tw<N, R1, Lay>(x, l, t, wk, wre, wim);
+            if (!FIRST && !a.do_fwd) continue;
+            if (PER) pfirst_fwd_2l<N, R1, Lay>(x[0], x[NR - 1], l, t, wk, wre, wim);
+            else pfirst_fwd_tw<N, R1, Lay>(x[0], l, t, wk, wre, wim);
         }
         group_sync<GT>(g);
         const int gt_next = FIRST ? gt + gstride : next_gt[g];
@@ -431,10 +464,19 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 #pragma unroll
             for (int j = 0; j < RL; ++j) v[j] = lds_p2(wk + Lay::addr(l, b * RL + j));
             pbfly<RL, -1>(v);
-            float4 *gp = reinterpret_cast<float4 *>(a.W + (long long)row * M) + b;
+            if (PER) {
+                float2 *ga = a.W + (long long)row * M + b;
 #pragma unroll
-            for (int i = 0; i < RL; ++i)
-                gp[brev(i, RL) * NBL] = make_float4(v[i].re.x, v[i].im.x, v[i].re.y, v[i].im.y);
+                for (int i = 0; i < RL; ++i) {
+                    ga[brev(i, RL) * NBL] = make_float2(v[i].re.x, v[i].im.x);
+                    ga[N + brev(i, RL) * NBL] = make_float2(v[i].re.y, v[i].im.y);
+                }
+            } else {
+                float4 *gp = reinterpret_cast<float4 *>(a.W + (long long)row * M) + b;
+#pragma unroll
+                for (int i = 0; i < RL; ++i)
+                    gp[brev(i, RL) * NBL] = make_float4(v[i].re.x, v[i].im.x, v[i].re.y, v[i].im.y);
+            }
         }
         if (FIRST) group_sync<GT>(g);  // the next tile's first stage writes slots other threads still read
         gt = gt_next;
@@ -501,34 +543,40 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 // tile buffer used in place for both directions; the last inverse stage of a tile is fused with the
 // first forward stage of the next one (as in k_row), so a tile costs four stages and ONE CTA-wide
 // barrier; between them the T line groups run on their own barriers.
-template <int N, int T, int MINB, bool KABS>
-__global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
+//
+// PER = true: the periodic (unpadded) form of the paper itself (Eq. 19, Alg. 1 l.36-38): one
+// length-N transform per column, and the two lanes of every packed value are the two columns of a 16-byte chunk
+// of the tile -- T/2 line slots per tile, the tile buffer read and written 16 bytes at a time, half the columns
+// and half the arithmetic per column of the padded form.  2-D only (a.p2_outer is not read).
+template <int N, int T, int MINB, bool KABS, bool PER = false>
+__global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
     constexpr int S1 = N / R1;
     constexpr int TPL = tpl_of(N);
-    constexpr int NT = T * TPL;
+    constexpr int NL = PER ? T / 2 : T;  // line slots of a tile
+    constexpr int NT = NL * TPL;
     constexpr int GT = TPL >= 32 ? TPL : 32;
     static_assert(T % 2 == 0 && NT % 32 == 0, "tile shape");
     constexpr int CPR = T / 2;  // 16-byte chunks (line pairs) per position
     constexpr bool WL = warp_local_mid(R2, RL, TPL);  // see k_row
     // fused last/first stage by line pairs (see there): when the stage has an item for every thread of two lines
-    constexpr bool PAIRX = conv_pair_exchange(N) && (2 * TPL) % 32 == 0 && T / 2 <= 7;
+    constexpr bool PAIRX = !PER && conv_pair_exchange(N) && (2 * TPL) % 32 == 0 && T / 2 <= 7;
     using Lay = LineLay<N>;
     extern __shared__ __align__(1024) float2 sm[];
     float4 *wk = reinterpret_cast<float4 *>(sm);  // [T][PITCH] work area, both halves per slot
     // Staged input tile, position-major like global memory: [N][CPR] chunks of 16 bytes (lines 2c,
     // 2c+1), the chunk index XOR-swizzled with the position (the TMA swizzle mode of that row width)
     // so that the 8-byte reads of a line group (consecutive positions) are 2-way at worst.
-    float4 *stg = wk + conv_stage_offset(N, T) / 16;  // 1024-byte aligned (TMA swizzle atom)
+    float4 *stg = wk + conv_stage_offset(N, NL) / 16;  // 1024-byte aligned (TMA swizzle atom)
     __shared__ __align__(8) uint64_t mbar;
     // Shared-memory copies of the tables every tile re-reads, for the tile shapes that leave room
     // (fft_engine.cuh, conv_p2_in_smem): the middle-stage twiddles C and the line-axis spectrum table.
-    constexpr bool P2SM = conv_p2_in_smem(N, T);
+    constexpr bool P2SM = !PER && conv_p2_in_smem(N, T);
     float2 *lutC_s = reinterpret_cast<float2 *>(stg + N * CPR);
     float2 *p2_s = lutC_s + (R2 > 0 ? S1 : 0);
-    if (a.ctl->done) return;
+    griddep_launch();
 
     const int tid = threadIdx.x;
     const int line = tid / TPL, lt = tid % TPL;
@@ -558,6 +606,9 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     const float2 *p2_tab = P2SM ? p2_s : a.p2_line;
     const float2 *lutC_tab = P2SM ? lutC_s : a.lut.C;
     __syncthreads();
+    // everything above reads plan constants only; the tiles and the stop flag are the previous kernel's
+    griddep_wait();
+    if (a.ctl->done) return;
     // I/O element of this thread's line at position r of the tile buffer
     float2 *io = reinterpret_cast<float2 *>(stg) + (line & 1);
     auto io_at = [&](int r) -> float2 & { return io[2 * (r * CPR + ((line >> 1) ^ swz(r)))]; };
@@ -580,10 +631,23 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
     phase ^= 1u;
 #pragma unroll 1
     for (int t = lt; t < S1; t += TPL) {
-        float2 x[R1];
+        if (PER) {
+            float2 wre[R1], wim[R1], xa[R1], xb[R1];
+            load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
 #pragma unroll
-        for (int j = 0; j < R1; ++j) x[j] = io_at(t + j * S1);
-        pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
+            for (int j = 0; j < R1; ++j) {
+                const int r = t + j * S1;
+                const float4 f = stg[r * CPR + (line ^ swz(r))];
+                xa[j] = make_float2(f.x, f.y);
+                xb[j] = make_float2(f.z, f.w);
+            }
+            pfirst_fwd_2l<N, R1, Lay>(xa, xb, line, t, wk, wre, wim);
+        } else {
+            float2 x[R1];
+#pragma unroll
+            for (int j = 0; j < R1; ++j) x[j] = io_at(t + j * S1);
+            pfirst_fwd<N, R1, Lay>(x, line, t, wk, a.lut.AB);
+        }
     }
     __syncthreads();
     int to_load = tile + 2 * (int)gridDim.x < total ? tile + 2 * (int)gridDim.x : -1;  // refill after the next store
@@ -603,8 +667,8 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         };
         auto line_alpha = [&](int in0, int out) { return line_alpha_of(in0, out, line); };
         float a_line = 0.f;
-        if (KABS) a_line = line_alpha(inner0, outer);
-        const bool dead = KABS && a_line > 1.0e17f;
+        if (KABS && !PER) a_line = line_alpha(inner0, outer);
+        const bool dead = KABS && !PER && a_line > 1.0e17f;
         if (R2 > 0) {
             if (!dead) pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
             if (WL) __syncwarp();
@@ -618,10 +682,14 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
         }
         if (!dead) {
             if (!KABS) a_line = line_alpha(inner0, outer);
+            float2 a_line2 = f2(a_line);
+            // periodic form: the slot's two columns; the x table holds the N-grid value at entries 2q and 2q + 1
+            if (PER) a_line2 = make_float2((__ldg(&a.p2_inner[2 * (inner0 + 2 * line)]) - 1.0f) * a.inv_e,
+                                           (__ldg(&a.p2_inner[2 * (inner0 + 2 * line + 1)]) - 1.0f) * a.inv_e);
             KAbs ka = a.kabs;
             if (KABS && a.ctl->term == 0) ka.nu = 0.f;  // term 0 is u_0 = A G S: the plain Green's spectrum
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line, ka);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line2, ka);
         }
         if (WL) __syncwarp();
         else group_sync<GT>(g);
@@ -637,11 +705,29 @@ __global__ void __launch_bounds__(T * tpl_of(N), MINB) k_conv(ColArgs a, const _
             phase ^= 1u;
         }
         bool dead_next = false;  // the same line of the next tile (another outer index in 3-D)
-        if (KABS && more) {
+        if (KABS && !PER && more) {
             const int nt = tile + (int)gridDim.x;
             dead_next = line_alpha((nt % tiles) * T, nt / tiles) > 1.0e17f;
         }
-        if (PAIRX) {
+        if (PER) {
+#pragma unroll 1
+            for (int t = lt; t < S1; t += TPL) {
+                float2 wre[R1], wim[R1];
+                load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
+                float2 za[R1], zb[R1], xa[R1], xb[R1];
+                plast_inv_2l<N, R1, Lay>(za, zb, line, t, wk, wre, wim);
+#pragma unroll
+                for (int j = 0; j < R1; ++j) {
+                    const int r = t + j * S1;
+                    float4 &e = stg[r * CPR + (line ^ swz(r))];
+                    const float4 f = e;
+                    xa[j] = make_float2(f.x, f.y);
+                    xb[j] = make_float2(f.z, f.w);
+                    e = make_float4(za[j].x, za[j].y, zb[j].x, zb[j].y);
+                }
+                if (more) pfirst_fwd_2l<N, R1, Lay>(xa, xb, line, t, wk, wre, wim);
+            }
+        } else if (PAIRX) {
             // Pair exchange: a thread does this stage for BOTH lines of a 16-byte chunk of the tile buffer at its
             // positions, so the buffer is read and written 16 bytes at a time (conflict-free under the TMA swizzle,
             // half the instructions of the per-line 8-byte exchange) and the twiddles are fetched once per pair.

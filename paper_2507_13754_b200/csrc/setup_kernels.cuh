@@ -22,7 +22,8 @@ __global__ void k_stage_lut(float2 *lut, int L, int R, int which) {
 
 // First/last-stage tables A and B interleaved for the packed engine (fft_engine_x2.cuh):
 // lut[k][t] = (A.x, B.x, A.y, B.y), A = exp(-2 pi i k t / N), B = exp(-2 pi i (2k+1) t / (2N)).
-__global__ void k_stage_lut_ab(float4 *lut, int N, int R) {
+// same_lanes = 1 (periodic, unpadded form: both lanes are whole lines): B = A.
+__global__ void k_stage_lut_ab(float4 *lut, int N, int R, int same_lanes) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int S = N / R;
     if (i >= S * R) return;
@@ -30,6 +31,7 @@ __global__ void k_stage_lut_ab(float4 *lut, int N, int R) {
     double sa, ca, sb, cb;
     sincospi(-2.0 * (double)((long long)k * t % N) / (double)N, &sa, &ca);
     sincospi(-2.0 * (double)((long long)(2 * k + 1) * t % (2 * N)) / (double)(2 * N), &sb, &cb);
+    if (same_lanes) { cb = ca; sb = sa; }
     lut[i] = make_float4((float)ca, (float)cb, (float)sa, (float)sb);
 }
 
@@ -74,6 +76,15 @@ __global__ void k_axis_table(float *p2, int N, int r1, int r2, int rl, double dx
     const double p = 2.0 * 3.14159265358979323846 * Ft / ((double)M * dx);
     // periodic boundary: only the even padded frequencies F = 2k exist (they are the frequencies of the
     // unpadded N-grid); an entry of 1e18 makes ghat vanish (to 1e-18) at the odd ones in every kernel
+    // periodic = 2 (unpadded periodic kernels): entries 2q and 2q + 1 both hold the N-grid value of frequency q,
+    // which is the padded grid's even frequency 2q
+    if (periodic == 2) {
+        const int Fe = F & ~1;
+        const double Fte = (Fe < M / 2) ? (double)Fe : (double)(Fe - M);
+        const double pe = 2.0 * 3.14159265358979323846 * Fte / ((double)M * dx);
+        p2[P] = (float)((pe * pe) / (k0 * k0) * mult);
+        return;
+    }
     p2[P] = (periodic && s == 1) ? 1.0e18f : (float)((p * p) / (k0 * k0) * mult);
 }
 

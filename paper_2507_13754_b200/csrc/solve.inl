@@ -11,10 +11,12 @@ tbs_status build_graph(tbs_plan *pl, Freq &f, int si, int half, int batch) {
     cudaStream_t cs;
     CU(pl, cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     cudaGraph_t g = nullptr;
-    const int sm_limit = half ? (pl->sms + 1) / 2 : 0;
+    LaunchOpt opt;
+    opt.sm_limit = half ? (pl->sms + 1) / 2 : 0;
+    opt.overlap = pl->overlap != 0;
     cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
     if (e == cudaSuccess) {
-        for (int i = 0; i < batch && e == cudaSuccess; ++i) e = launch_term(pl, f, pl->slot[si], cs, sm_limit);
+        for (int i = 0; i < batch && e == cudaSuccess; ++i) e = launch_term(pl, f, pl->slot[si], cs, opt);
         cudaError_t e2 = cudaStreamEndCapture(cs, &g);
         if (e == cudaSuccess) e = e2;
     }
@@ -60,7 +62,9 @@ tbs_status run_begin(tbs_plan *pl, Run &r, int ifreq, int si, cudaStream_t st, i
     // term 0 forward half: W = FFT_x(pad(S / k0^2))
     RowArgs ra;
     fill_row_args(pl, f, s, ra, f.S, (float)(1.0 / (f.k0 * f.k0)), 1);
-    CU(pl, launch_row(pl->n[0], true, ra, st, false, half ? (pl->sms + 1) / 2 : 0));
+    LaunchOpt opt;
+    opt.sm_limit = half ? (pl->sms + 1) / 2 : 0;
+    CU(pl, launch_row(pl->n[0], true, ra, st, false, opt));
     pl->launches += 1;
     return TBS_OK;
 }
@@ -75,7 +79,10 @@ tbs_status run_enqueue(tbs_plan *pl, Run &r) {
         if (gs != TBS_OK) return gs;
         CU(pl, cudaGraphLaunch(f.graph[r.si][r.half].exec, r.st));
     } else {
-        for (int i = 0; i < batch; ++i) CU(pl, launch_term(pl, f, s, r.st, r.half ? (pl->sms + 1) / 2 : 0));
+        LaunchOpt opt;
+        opt.sm_limit = r.half ? (pl->sms + 1) / 2 : 0;
+        opt.overlap = pl->overlap != 0;
+        for (int i = 0; i < batch; ++i) CU(pl, launch_term(pl, f, s, r.st, opt));
     }
     pl->launches += (long long)batch * (mid_launches(pl) + 1);
     CU(pl, cudaMemcpyAsync(&s.h_ctl[1 + (r.issued & 1)], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, r.st));
@@ -361,11 +368,13 @@ tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4],
     fill_row_args(pl, f, s, r, nullptr, 0.f, 1);
     for (int k = 0; k < 4; ++k) out_ms[k] = 0.0;
     tbs_status res = TBS_OK;
+    LaunchOpt popt;
+    popt.overlap = pl->overlap != 0;
     // out_ms[0] = row kernel, out_ms[1..] = column/plane passes in launch order
     for (int k = 0; k <= nmid && res == TBS_OK; ++k) {
         cudaError_t e = cudaEventRecord(pl->ev_b0, st);
         for (int i = 0; i < reps && e == cudaSuccess; ++i)
-            e = k < nmid ? launch_mid_passes(pl, f, s, st, k) : launch_row(pl->n[0], false, r, st);
+            e = k < nmid ? launch_mid_passes(pl, f, s, st, k, popt) : launch_row(pl->n[0], false, r, st, false, popt);
         if (e == cudaSuccess) e = cudaEventRecord(pl->ev_b1, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         float ms = 0.f;

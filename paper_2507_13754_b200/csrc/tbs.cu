@@ -82,6 +82,7 @@ struct tbs_plan {
     size_t small_bytes = 0;      // device bytes outside the workspace (tables, control)
     int graph_batch = 16;
     int concurrency = kMaxSlots;
+    int overlap = 0;             // programmatic dependent launch of the term kernels (measured slower: off)
     int scheme = TBS_SCHEME_BORN;
     int boundary = TBS_BOUNDARY_PAD;
     int crit_row = -1;
@@ -124,6 +125,10 @@ bool pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 inline unsigned nblk(long long n, int b) { return (unsigned)((n + b - 1) / b); }
 inline size_t align_up(size_t v) { return (v + kWsAlign - 1) / kWsAlign * kWsAlign; }
 
+// Periodic boundary in 2-D: the unpadded kernels (one N-point transform per line, W1 is [ny][nx]); in 3-D the
+// padded kernels with masked axis tables.
+bool per_mode(const tbs_plan *pl) { return pl->boundary == TBS_BOUNDARY_PERIODIC && pl->ndim == 2; }
+
 size_t w1_elems(const tbs_plan *pl) { return (size_t)pl->n[1] * pl->n[2] * 2 * pl->n[0]; }
 size_t w2_elems(const tbs_plan *pl) { return pl->ndim == 3 ? (size_t)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0] : 0; }
 
@@ -157,6 +162,19 @@ void destroy_graphs(tbs_plan *pl) {
             }
 }
 
+// Tensor maps of the arrays k_conv transforms in place: W1 ([ny][2 nx], or [ny][nx] in the unpadded periodic
+// form) in 2-D, W2 in 3-D.
+tbs_status make_tensor_maps(tbs_plan *pl) {
+    if (!pl->ws) return TBS_OK;
+    const long long mx = (per_mode(pl) ? 1LL : 2LL) * pl->n[0], my = 2LL * pl->n[1];
+    for (int i = 0; i < pl->nslots; ++i) {
+        Slot &s = pl->slot[i];
+        if (pl->ndim == 2) CU(pl, make_conv_tensor_map(&s.conv_map, s.W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
+        else CU(pl, make_conv_tensor_map(&s.conv_map, s.W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
+    }
+    return TBS_OK;
+}
+
 // Point the plan at a workspace.  Its contents are undefined: medium and source have to be set (again).
 tbs_status bind_workspace(tbs_plan *pl, void *base, size_t bytes, bool owned) {
     destroy_graphs(pl);
@@ -166,13 +184,7 @@ tbs_status bind_workspace(tbs_plan *pl, void *base, size_t bytes, bool owned) {
     pl->ws_owned = owned;
     workspace_layout(pl, (char *)base, true);
     for (auto &f : pl->fr) { f.have_V = false; f.have_S = false; }
-    const long long mx = 2LL * pl->n[0], my = 2LL * pl->n[1];
-    for (int i = 0; i < pl->nslots; ++i) {
-        Slot &s = pl->slot[i];
-        if (pl->ndim == 2) CU(pl, make_conv_tensor_map(&s.conv_map, s.W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
-        else CU(pl, make_conv_tensor_map(&s.conv_map, s.W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
-    }
-    return TBS_OK;
+    return make_tensor_maps(pl);
 }
 
 // Every call that touches V, S, p or W goes through here: without a caller-owned workspace the plan allocates.
@@ -201,6 +213,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, Slot &s, RowArgs &a, const float2 *src
     a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
     if (pl->boundary == TBS_BOUNDARY_PERIODIC) a.scale *= (float)(1 << pl->ndim);  // the odd half carries nothing
     a.do_fwd = do_fwd;
+    a.per = per_mode(pl);
     a.norms = s.norms;
     a.history = s.history;
     a.ctl = f.ctl;
@@ -208,15 +221,16 @@ void fill_row_args(tbs_plan *pl, Freq &f, Slot &s, RowArgs &a, const float2 *src
 }
 
 // Column / plane passes of one term (K2 in 2-D; y-forward, z-conv, y-inverse in 3-D).
-cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int which = -1, int sm_limit = 0) {
+cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int which = -1, LaunchOpt opt = LaunchOpt()) {
     const int nx = pl->n[0], ny = pl->n[1], nz = pl->n[2];
-    const long long mx = 2LL * nx, my = 2LL * ny;
+    const long long mx = (per_mode(pl) ? 1LL : 2LL) * nx, my = 2LL * ny;
     ColArgs a;
     memset(&a, 0, sizeof a);
     a.ctl = f.ctl;
     a.inv_e = (float)(1.0 / pl->damping);
     a.kabs = f.kabs;
-    a.masked = pl->boundary == TBS_BOUNDARY_PERIODIC;
+    a.per = per_mode(pl);
+    a.masked = pl->boundary == TBS_BOUNDARY_PERIODIC && !a.per;
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
     if (pl->ndim == 2) {
@@ -224,7 +238,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, i
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = a.out_line_stride = mx;
         a.p2_line = (const float2 *)f.p2[1]; a.p2_inner = f.p2[0]; a.p2_outer = nullptr;
-        if (which < 0 || which == 0) e = launch_conv(ny, a, &s.conv_map, 1, st, false, sm_limit);
+        if (which < 0 || which == 0) e = launch_conv(ny, a, &s.conv_map, 1, st, false, opt);
         return e;
     }
     // y forward: W1[z][y][kx] -> W2[z][ky][kx]
@@ -233,7 +247,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, i
         a.lut = Luts{pl->lutA[1], pl->lutB[1], pl->lutC[1], pl->lutAB[1]};
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = (long long)ny * mx; a.out_outer_stride = my * mx;
-        e = launch_col(ny, MODE_FWD, a, nz, st, false, sm_limit);
+        e = launch_col(ny, MODE_FWD, a, nz, st, false, opt);
         if (e != cudaSuccess) return e;
     }
     // z convolution, in place on W2; lines (ky, kx), outer = ky
@@ -243,7 +257,7 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, i
         a.in_line_stride = a.out_line_stride = my * mx;
         a.in_outer_stride = a.out_outer_stride = mx;
         a.p2_line = (const float2 *)f.p2[2]; a.p2_inner = f.p2[0]; a.p2_outer = f.p2[1];
-        e = launch_conv(nz, a, &s.conv_map, (int)my, st, false, sm_limit);
+        e = launch_conv(nz, a, &s.conv_map, (int)my, st, false, opt);
         if (e != cudaSuccess) return e;
     }
     // y inverse: W2[z][ky][kx] -> W1[z][y][kx]
@@ -253,19 +267,19 @@ cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, i
         a.in_line_stride = mx; a.out_line_stride = mx;
         a.in_outer_stride = my * mx; a.out_outer_stride = (long long)ny * mx;
         a.p2_line = nullptr; a.p2_inner = nullptr; a.p2_outer = nullptr;
-        e = launch_col(ny, MODE_INV, a, nz, st, false, sm_limit);
+        e = launch_col(ny, MODE_INV, a, nz, st, false, opt);
     }
     return e;
 }
 
 int mid_launches(const tbs_plan *pl) { return pl->ndim == 2 ? 1 : 3; }
 
-cudaError_t launch_term(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int sm_limit = 0) {
-    cudaError_t e = launch_mid_passes(pl, f, s, st, -1, sm_limit);
+cudaError_t launch_term(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, LaunchOpt opt = LaunchOpt()) {
+    cudaError_t e = launch_mid_passes(pl, f, s, st, -1, opt);
     if (e != cudaSuccess) return e;
     RowArgs r;
     fill_row_args(pl, f, s, r, nullptr, 0.f, 1);
-    return launch_row(pl->n[0], false, r, st, false, sm_limit);
+    return launch_row(pl->n[0], false, r, st, false, opt);
 }
 
 // Green's-spectrum axis tables of one frequency, in the order each kernel reads them (setup_kernels.cuh).
@@ -276,7 +290,7 @@ cudaError_t fill_axis_tables(tbs_plan *pl, Freq &f) {
         k_axis_table<<<nblk(2 * pl->n[a], 256), 256>>>(f.p2[a], pl->n[a], r1, r2, rl, pl->dx, f.k0,
                                                         a == 0 || a == pl->ndim - 1,
                                                         a == pl->ndim - 1 ? 1.0 / pl->damping : 1.0,
-                                                        pl->boundary == TBS_BOUNDARY_PERIODIC);
+                                                        per_mode(pl) ? 2 : pl->boundary == TBS_BOUNDARY_PERIODIC);
     }
     return cudaGetLastError();
 }
@@ -368,6 +382,13 @@ tbs_status tbs_set_graph_batch(tbs_plan *plan, int terms_per_graph) {
     return TBS_OK;
 }
 
+tbs_status tbs_set_launch_overlap(tbs_plan *plan, int on) {
+    if (!plan) return TBS_ERR_INVALID_ARG;
+    plan->overlap = on ? 1 : 0;
+    destroy_graphs(plan);
+    return TBS_OK;
+}
+
 tbs_status tbs_set_concurrency(tbs_plan *plan, int members) {
     if (!plan || members < 1 || members > kMaxSlots) return TBS_ERR_INVALID_ARG;
     plan->concurrency = members;
@@ -439,7 +460,7 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
             k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutA[a], N, r1, 0);
             k_stage_lut<<<nblk(N, 256), 256>>>(pl->lutB[a], N, r1, 1);
             CU(pl, dmalloc(pl, &pl->lutAB[a], N));
-            k_stage_lut_ab<<<nblk(N, 256), 256>>>(pl->lutAB[a], N, r1);
+            k_stage_lut_ab<<<nblk(N, 256), 256>>>(pl->lutAB[a], N, r1, 0);
             if (r2 > 0) {
                 CU(pl, dmalloc(pl, &pl->lutC[a], N / r1));
                 k_stage_lut<<<nblk(N / r1, 256), 256>>>(pl->lutC[a], N / r1, r2, 0);
@@ -524,8 +545,18 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
 
 tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
     if (!pl || (boundary != TBS_BOUNDARY_PAD && boundary != TBS_BOUNDARY_PERIODIC)) return TBS_ERR_INVALID_ARG;
+    CU(pl, cudaDeviceSynchronize());
     pl->boundary = boundary;
     for (auto &f : pl->fr) CU(pl, fill_axis_tables(pl, f));
+    // first/last-stage twiddles: the odd lane carries the padding twist, or (unpadded periodic form) a second line
+    for (int a = 0; a < pl->ndim; ++a) {
+        int r1, r2, rl;
+        radices_of(pl->n[a], r1, r2, rl);
+        k_stage_lut_ab<<<nblk(pl->n[a], 256), 256>>>(pl->lutAB[a], pl->n[a], r1, per_mode(pl) ? 1 : 0);
+    }
+    CU(pl, cudaGetLastError());
+    tbs_status ms = make_tensor_maps(pl);
+    if (ms != TBS_OK) return ms;
     destroy_graphs(pl);  // the captured launches carry the normalisation
     CU(pl, cudaDeviceSynchronize());
     return TBS_OK;

@@ -113,6 +113,10 @@ class Plan:
     def device_bytes(self):
         return int(self._L.tbs_plan_device_bytes(self._h))
 
+    def set_launch_overlap(self, on):
+        """tbs_set_launch_overlap: programmatic dependent launch of the term kernels (default on)."""
+        self._check(self._L.tbs_set_launch_overlap(self._h, int(bool(on))))
+
     def set_concurrency(self, members):
         """tbs_set_concurrency: members of a frequency batch solved at once (1 or 2)."""
         self._check(self._L.tbs_set_concurrency(self._h, int(members)))
