@@ -222,7 +222,7 @@ __host__ __device__ constexpr bool conv_p2_in_smem(int N, int T) {
     return conv_stage_offset(N, T) + N * T * 8 + conv_lutc_entries(N) * 8 + N * 8 <= 128 * 1024;
 }
 __host__ __device__ constexpr int conv_smem_bytes(int N, int T) {
-    return conv_stage_offset(N, T) + N * T * 8 + (conv_p2_in_smem(N, T) ? conv_lutc_entries(N) * 8 + N * 8 : 0);
+    return conv_stage_offset(N, T) + N * T * 8 + conv_lutc_entries(N) * 8 + (conv_p2_in_smem(N, T) ? N * 8 : 0);
 }
 // the periodic form of k_conv (T/2 line slots per tile, no table copies)
 __host__ __device__ constexpr int conv_smem_bytes_per(int N, int T) { return conv_stage_offset(N, T / 2) + N * T * 8; }

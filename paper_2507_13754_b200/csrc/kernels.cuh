@@ -574,8 +574,9 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
     // Shared-memory copies of the tables every tile re-reads, for the tile shapes that leave room
     // (fft_engine.cuh, conv_p2_in_smem): the middle-stage twiddles C and the line-axis spectrum table.
     constexpr bool P2SM = !PER && conv_p2_in_smem(N, T);
+    constexpr bool CSM = !PER && R2 > 0;  // the middle-stage table is small (N/R1 entries): always copied
     float2 *lutC_s = reinterpret_cast<float2 *>(stg + N * CPR);
-    float2 *p2_s = lutC_s + (R2 > 0 ? S1 : 0);
+    float2 *p2_s = lutC_s + conv_lutc_entries(N);
     griddep_launch();
 
     const int tid = threadIdx.x;
@@ -598,13 +599,12 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
         for (int k = 0; k < N / BR; ++k) tma_load_2d(stg + k * BR * CPR, &tmap, c0, k * BR, &mbar);
     };
     if (tid == 0) mbar_init(&mbar, 1);
-    if (P2SM) {
-        if (R2 > 0)
-            for (int i = tid; i < S1; i += NT) lutC_s[i] = __ldg(a.lut.C + i);
+    if (CSM)
+        for (int i = tid; i < S1; i += NT) lutC_s[i] = __ldg(a.lut.C + i);
+    if (P2SM)
         for (int i = tid; i < N; i += NT) p2_s[i] = __ldg(a.p2_line + i);
-    }
     const float2 *p2_tab = P2SM ? p2_s : a.p2_line;
-    const float2 *lutC_tab = P2SM ? lutC_s : a.lut.C;
+    const float2 *lutC_tab = CSM ? lutC_s : a.lut.C;
     __syncthreads();
     // everything above reads plan constants only; the tiles and the stop flag are the previous kernel's
     griddep_wait();
@@ -670,7 +670,7 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
         if (KABS && !PER) a_line = line_alpha(inner0, outer);
         const bool dead = KABS && !PER && a_line > 1.0e17f;
         if (R2 > 0) {
-            if (!dead) pstage_line<N, S1, R2s, true, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
+            if (!dead) pstage_line<N, S1, R2s, true, Lay, TPL, CSM>(wk, lutC_tab, line, lt);
             if (WL) __syncwarp();
             else group_sync<GT>(g);  // by every line: lines of different state may share a warp
             // by now the store of the previous tile has been read out of the buffer: refill it
@@ -694,7 +694,7 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
         if (WL) __syncwarp();
         else group_sync<GT>(g);
         if (R2 > 0) {
-            if (!dead) pstage_line<N, S1, R2s, false, Lay, TPL, P2SM>(wk, lutC_tab, line, lt);
+            if (!dead) pstage_line<N, S1, R2s, false, Lay, TPL, CSM>(wk, lutC_tab, line, lt);
             if (!PAIRX) group_sync<GT>(g);
         }
         // pair exchange: the next stage reads both lines of the thread's pair
