@@ -580,7 +580,13 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
     griddep_launch();
 
     const int tid = threadIdx.x;
-    const int line = tid / TPL, lt = tid % TPL;
+    // Two lines per warp (TPL = 16): quarter-warps alternate between the lines, so that the 8-byte accesses of a
+    // half-warp to the tile buffer (lines 2c, 2c + 1 at 8 consecutive positions) fill whole 16-byte chunks --
+    // conflict-free, where 16 positions of one line are 2-way.  The 16-byte work-area accesses go by quarter-warp
+    // and see the same pattern either way.
+    constexpr bool QW = TPL == 16 && !PER;
+    const int line = QW ? (tid >> 5) * 2 + ((tid >> 3) & 1) : tid / TPL;
+    const int lt = QW ? (tid & 7) + ((tid >> 4) & 1) * 8 : tid % TPL;
     const int g = tid / GT;
     const int tiles = a.inner_len / T;
     const int total = tiles * a.n_outer;
