@@ -179,3 +179,23 @@ def test_frequency_batch_solved_together_matches_per_frequency_oracle(maker, kw,
         compare_fields(res.p[i].cpu().numpy(), ref.p, f"{w.name} member {i}")
         n = min(int(res.n_terms[i]), ref.n_terms)
         compare_history(res.history[i], ref.history, n, rtol=2e-3)
+
+
+# ------------------------------------------------------------------ launch switches do not change results
+def test_launch_overlap_and_plain_launches_give_the_same_series():
+    """tbs_set_launch_overlap (programmatic dependent launch: every kernel orders its memory accesses behind its
+    predecessor with griddepcontrol.wait) and tbs_set_graph_batch(0) (no CUDA graph) change how the kernels of a
+    term are launched, not what they compute."""
+    for w in (W.cfg3(N=256), W.cfg5(N=32)):
+        base = gpu_plan(w).solve(w.max_terms, w.tol)
+        assert base.status == 0
+        for setup in ("overlap", "nograph", "overlap+nograph"):
+            plan = gpu_plan(w)
+            if "overlap" in setup:
+                plan.set_launch_overlap(True)
+            if "nograph" in setup:
+                plan.set_graph_batch(0)
+            res = plan.solve(w.max_terms, w.tol)
+            assert res.status == 0 and int(res.n_terms[0]) == int(base.n_terms[0]), setup
+            assert float((res.p - base.p).abs().max() / base.p.abs().max()) < 1e-5, setup
+            assert np.allclose(res.history, base.history, rtol=1e-5), setup
