@@ -53,8 +53,32 @@ def test_periodic_boundary_matches_oracle_pad_factor_one():
     compare_fields(res.p[0].cpu().numpy(), ref.p, "periodic 128^2")
 
 
+@pytest.mark.parametrize("shape", [(32, 32), (64, 128), (128, 64), (256, 256), (512, 1024), (1024, 32), (32, 1024),
+                                   (2048, 64), (64, 2048), (4096, 32), (32, 4096), (2048, 2048)])
+def test_unpadded_periodic_kernels_apply_green_every_length(shape):
+    """The unpadded kernels (k_row / k_conv <..., PER>: two lines per packed value) at every transform length in
+    both axes: one application of G on the periodic N-grid against the oracle's pad-factor-1 definition."""
+    from paper_2507_13754_b200.tbs import Plan
+    rng = np.random.default_rng(sum(shape) + 1)
+    x = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    dx = 1500.0 / 1.0e6 / 6.0
+    plan = Plan(shape, dx, [1.0e6], 1500.0, 0.8)
+    plan.set_boundary("periodic")
+    out = plan.apply_green(0, torch.from_numpy(x).cuda()).cpu().numpy()
+    k0, eps = R.wavenumber(1.0e6, 1500.0, 0.8)
+    ref = R.apply_G(x.astype(np.complex128), R.green_spectrum(shape, dx, k0, eps), 1)
+    rel = np.linalg.norm(out - ref) / np.linalg.norm(ref)
+    assert rel < 2e-6, rel
+    # switching back to the padded boundary on the same plan restores the linear convolution
+    plan.set_boundary("pad")
+    if max(shape) <= 1024:
+        out2 = plan.apply_green(0, torch.from_numpy(x).cuda()).cpu().numpy()
+        ref2 = R.apply_G(x.astype(np.complex128), R.green_spectrum(tuple(2 * s for s in shape), dx, k0, eps))
+        assert np.linalg.norm(out2 - ref2) / np.linalg.norm(ref2) < 2e-6
+
+
 def test_periodic_boundary_512_matches_oracle_pad_factor_one():
-    """N = 512: a line is owned by a whole warp, so k_conv skips the masked (odd-frequency) columns outright."""
+    """N = 512, 40 terms with the absorbing layer, history term by term."""
     N, abl = 512, 32
     case = _case(N, abl)
     V, S, g, win = _oracle_inputs(N, abl, *case)
