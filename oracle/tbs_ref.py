@@ -293,9 +293,13 @@ def kspace_potential(shape_padded, dx: float, alpha0_si: float, nu: float, f_hz:
     return -1j * tau * w * k ** nu + eta * k ** (nu + 1.0) - 1j * eps
 
 
-def solve_kspace(S, ghat, VV, max_terms: int, tol: float, pad: int = 2, windows=None, row=None) -> RefResult:
+def solve_kspace(S, ghat, VV, max_terms: int, tol: float, pad: int = 2, windows=None, row=None, Us=None) -> RefResult:
     """Eq. 24 in term form: u_0 = A G S, u_{n+1} = A F^-1[ghat VV F[u_n]], p = sum u_n (the Picard iterates of
-    Eq. 24 are these partial sums).  row = None: r_n = ||u_n||_2/||p_n||_2; row = r: Eq. 30 on that row."""
+    Eq. 24 are these partial sums).  row = None: r_n = ||u_n||_2/||p_n||_2; row = r: Eq. 30 on that row.
+    Us (optional, same shape as S): a scatterer in the absorbing medium -- the potential of Eq. 23
+    plus the spatial term U_s(r) = k_s(r)^2 - k_f^2 of Eq. 25 (the -i eps is already in VV):
+    u_{n+1} = A F^-1[ghat (VV F[u_n] + F[U_s u_n])].  The paper runs the two potentials separately (Eq. 24, Eq. 26);
+    this is their sum, both being terms of the same operator V in psi = G V psi + G S (Eq. 17)."""
     S = np.ascontiguousarray(S, dtype=np.complex128)
     A = np.ones(S.shape)
     if windows is not None:
@@ -311,7 +315,10 @@ def solve_kspace(S, ghat, VV, max_terms: int, tol: float, pad: int = 2, windows=
     hist = [1.0]
     status, k = NOT_CONVERGED, 0
     for k in range(1, max_terms + 1):
-        u = A * apply_G(u, gv, pad)
+        if Us is None:
+            u = A * apply_G(u, gv, pad)
+        else:
+            u = A * (apply_G(u, gv, pad) + apply_G(Us * u, ghat, pad))
         if row is None:
             p += u
             r = math.sqrt(float(np.vdot(u, u).real)) / math.sqrt(float(np.vdot(p, p).real))

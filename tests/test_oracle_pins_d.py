@@ -197,3 +197,38 @@ def test_kspace_series_plane_wave_decays_with_the_power_law():
     dphi = np.unwrap(np.angle(res.p[0, a:b + 1]))
     Kre = (dphi[-1] - dphi[0]) / ((b - a) * dx)
     assert abs(Kre / K.real - 1) < 1e-3
+
+
+def test_kspace_potential_plus_scatterer_reduces_to_both_parents_and_to_the_typed_formula():
+    """solve_kspace(..., Us): (i) Us = 0 is Eq. 24 alone; (ii) a lossless multiplier VV = -i eps makes it the
+    ordinary series with V = U_s - i eps (Eq. 26); (iii) against the iteration typed with numpy's
+    FFT on the periodic grid: psi <- A ifft2(g (VV fft2(psi) + fft2(U_s psi + S)))  (Eq. 24 + the U_s term of Eq. 25)."""
+    N, dx, f, c0 = 32, 1.0e-4, 1.0e6, 1500.0
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    S = np.zeros((N, N), dtype=np.complex128)
+    S[10:22, 6] = -1.0e6j
+    yy, xx = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    Us = np.where((xx - 20) ** 2 + (yy - 15) ** 2 <= 16, (2 * np.pi * f / 1650.0) ** 2 - k0 * k0, 0.0).astype(np.complex128)
+    g = R.green_spectrum((N, N), dx, k0, eps)
+    VV = R.kspace_potential((N, N), dx, 5.5e-10 * 50, 1.5, f, c0, 0.8)
+    win = tuple(R.abl_window(N, 6) for _ in range(2))
+    A = np.outer(win[1], win[0])
+    # (i)
+    a = R.solve_kspace(S, g, VV, 25, 0.0, pad=1, windows=win)
+    b = R.solve_kspace(S, g, VV, 25, 0.0, pad=1, windows=win, Us=np.zeros_like(Us))
+    assert np.allclose(a.p, b.p, rtol=0, atol=1e-13 * np.abs(a.p).max()) and np.allclose(a.history, b.history)
+    # (ii)
+    lossless = np.full((N, N), -1j * eps)
+    c_ = R.solve_kspace(S, g, lossless, 25, 0.0, pad=1, windows=win, Us=Us)
+    d = R.solve(Us - 1j * eps, S, g, 25, 0.0, pad=1, windows=win)
+    assert np.allclose(c_.p, d.p, rtol=0, atol=1e-12 * np.abs(d.p).max()) and np.allclose(c_.history, d.history, rtol=1e-10)
+    # (iii) the Picard iterates typed out
+    res = R.solve_kspace(S, g, VV, 12, 0.0, pad=1, windows=win, Us=Us)
+    u = A * np.fft.ifft2(g * np.fft.fft2(S))
+    p = u.copy()
+    for _ in range(12):
+        u = A * np.fft.ifft2(g * (VV * np.fft.fft2(u) + np.fft.fft2(Us * u)))
+        p += u
+    assert np.abs(res.p - p).max() <= 1e-12 * np.abs(p).max()
+    # and the scatterer does change the field (the pin is not vacuous)
+    assert np.abs(res.p - R.solve_kspace(S, g, VV, 12, 0.0, pad=1, windows=win).p).max() > 1e-3 * np.abs(p).max()
