@@ -94,6 +94,17 @@ const char *tbs_last_error(const tbs_plan *plan);
  * forms are not combined).  With TBS_SCHEME_CBS selected (or selecting it afterwards): TBS_ERR_INVALID_ARG. */
 tbs_status tbs_set_kspace_absorption(tbs_plan *plan, double alpha0_si, double nu, int dispersive);
 
+/* A scatterer inside the absorbing(-dispersive) medium of tbs_set_kspace_absorption: the potential operator is the
+ * sum of the k-space multiplier of Eq. 23 and the spatial term U_s(r) = (w/c(r))^2 - k0^2 of Eq. 25
+ * (its -i eps is the multiplier's), so that
+ *   u_{n+1} = A F^-1[ghat(p) (VV(|p|) F[u_n] + F[U_s u_n])].
+ * The paper runs the two potentials in separate experiments (Eq. 24, Eq. 26); both are terms of the one operator V of
+ * Eq. 17.  c [n] dev float: sound-speed map (c == the plan's c0 outside the scatterer).  Needs the
+ * periodic boundary in 2-D (the paper's form: the unpadded kernels carry U_s u_n and u_n as the two lanes of every
+ * packed value and transform them together) and an active multiplier; else TBS_ERR_INVALID_ARG / TBS_ERR_NOT_READY.
+ * Undone by tbs_set_kspace_absorption, tbs_set_medium, tbs_set_potential or leaving the periodic boundary. */
+tbs_status tbs_set_kspace_scatterer(tbs_plan *plan, const float *c, void *stream);
+
 /* Boundary treatment (default TBS_BOUNDARY_PAD: zero-pad to 2N per axis, linear convolution, crop --
  * BASELINE north_star).  TBS_BOUNDARY_PERIODIC is the paper's own: the FFTs act on the N-grid itself
  * (Eq. 19, Alg. 1 l.36-38) and wrap-around is left to the absorbing layer of tbs_set_abl

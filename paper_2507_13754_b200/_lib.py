@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libtbs.so")
 SYMBOLS = [
     "tbs_version", "tbs_plan_create", "tbs_plan_destroy", "tbs_plan_workspace_bytes", "tbs_plan_set_workspace",
     "tbs_plan_device_bytes", "tbs_grid_harmonic_frequency", "tbs_set_concurrency", "tbs_set_launch_overlap", "tbs_last_error",
-    "tbs_set_abl", "tbs_set_scheme", "tbs_set_boundary", "tbs_set_criterion", "tbs_set_kspace_absorption", "tbs_set_medium", "tbs_set_medium_host", "tbs_set_potential", "tbs_set_source",
+    "tbs_set_abl", "tbs_set_scheme", "tbs_set_boundary", "tbs_set_criterion", "tbs_set_kspace_absorption", "tbs_set_kspace_scatterer", "tbs_set_medium", "tbs_set_medium_host", "tbs_set_potential", "tbs_set_source",
     "tbs_set_source_field", "tbs_solve", "tbs_solve_host", "tbs_solve_second_harmonic", "tbs_solve_harmonics",
     "tbs_apply_green", "tbs_get_potential", "tbs_get_source", "tbs_green_spectrum",
     "tbs_last_launch_count", "tbs_last_loop_ms", "tbs_profile_term", "tbs_set_graph_batch",
@@ -57,6 +57,7 @@ def load() -> ctypes.CDLL:
     L.tbs_set_scheme.argtypes = [vp, i32]
     L.tbs_set_boundary.argtypes = [vp, i32]
     L.tbs_set_kspace_absorption.argtypes = [vp, dbl, dbl, i32]
+    L.tbs_set_kspace_scatterer.argtypes = [vp, vp, vp]
     L.tbs_set_criterion.argtypes = [vp, i32, i32]
     L.tbs_set_medium.argtypes = [vp, vp, vp, vp, dbl, dbl, dbl, dbl, vp]
     L.tbs_set_medium_host.argtypes = [vp, vp, vp, vp, dbl, dbl, dbl, dbl, vp]

@@ -57,13 +57,13 @@ static cudaError_t launch_col_t(const ColArgs &a, int n_outer, cudaStream_t st, 
     return launch_k(kern, (unsigned)(total < cap ? total : cap), C::NT, smem, st, opt.overlap, b);
 }
 
-template <int N, bool KABS, bool PER = false>
+template <int N, bool KABS, bool PER = false, bool TWOF = false>
 static cudaError_t launch_conv_tt(const ColArgs &a, const CUtensorMap *tmap, int n_outer, cudaStream_t st, bool set_attr,
                                   LaunchOpt opt) {
     constexpr int T = ConvCfg<N>::T;
     constexpr int NT = (PER ? T / 2 : T) * tpl_of(N);
     constexpr size_t smem = PER ? (size_t)conv_smem_bytes_per(N, T) : (size_t)conv_smem_bytes(N, T);
-    auto kern = k_conv<N, T, ConvCfg<N>::MINB, KABS, PER>;
+    auto kern = k_conv<N, T, ConvCfg<N>::MINB, KABS, PER, TWOF>;
     static Resident res;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -77,7 +77,7 @@ static cudaError_t launch_conv_tt(const ColArgs &a, const CUtensorMap *tmap, int
     return launch_k(kern, (unsigned)(total < cap ? total : cap), NT, smem, st, opt.overlap, b, *tmap);
 }
 
-template <int N, bool FIRST, bool GEN, bool PER = false>
+template <int N, bool FIRST, bool GEN, bool PER = false, bool TWOF = false>
 static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_attr, LaunchOpt opt) {
     using C = RowCfg<N>;
     constexpr int TPL = row_tpl_of(N);
@@ -86,7 +86,7 @@ static cudaError_t launch_row_tt(const RowArgs &a, cudaStream_t st, bool set_att
     constexpr int ROWS = C::GROUPS * GR;
     constexpr size_t smem = 2 * (size_t)ROWS * LineLay<N>::PITCH * sizeof(float2) +
                             (FIRST || !row_staged(N) ? 0 : (size_t)ROWS * N * sizeof(float4));
-    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN, PER>;
+    auto kern = k_row<N, C::GROUPS, C::MINB, FIRST, GEN, PER, TWOF>;
     static Resident res;
     if (set_attr) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -106,8 +106,12 @@ cudaError_t launch_row_n(bool first, const RowArgs &a, cudaStream_t st, bool set
         if (e == cudaSuccess) e = launch_row_tt<N, false, true>(a, st, true, LaunchOpt());
         if (e == cudaSuccess) e = launch_row_tt<N, true, false, true>(a, st, true, LaunchOpt());
         if (e == cudaSuccess) e = launch_row_tt<N, false, true, true>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, true, false, false, true>(a, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_row_tt<N, false, true, false, true>(a, st, true, LaunchOpt());
         return e;
     }
+    if (a.per == 2) return first ? launch_row_tt<N, true, false, false, true>(a, st, false, opt)
+                                 : launch_row_tt<N, false, true, false, true>(a, st, false, opt);
     if (a.per) return first ? launch_row_tt<N, true, false, true>(a, st, false, opt)
                             : launch_row_tt<N, false, true, true>(a, st, false, opt);
     if (first) return launch_row_tt<N, true, false>(a, st, false, opt);
@@ -122,8 +126,10 @@ cudaError_t launch_conv_n(const ColArgs &a, const CUtensorMap *tmap, int n_outer
         cudaError_t e = launch_conv_tt<N, false>(a, tmap, n_outer, st, true, LaunchOpt());
         if (e == cudaSuccess) e = launch_conv_tt<N, true>(a, tmap, n_outer, st, true, LaunchOpt());
         if (e == cudaSuccess) e = launch_conv_tt<N, true, true>(a, tmap, n_outer, st, true, LaunchOpt());
+        if (e == cudaSuccess) e = launch_conv_tt<N, true, true, true>(a, tmap, n_outer, st, true, LaunchOpt());
         return e;
     }
+    if (a.per == 2) return launch_conv_tt<N, true, true, true>(a, tmap, n_outer, st, false, opt);
     if (a.per) return launch_conv_tt<N, true, true>(a, tmap, n_outer, st, false, opt);
     return a.kabs.nu > 0.f || a.masked ? launch_conv_tt<N, true>(a, tmap, n_outer, st, false, opt)
                                        : launch_conv_tt<N, false>(a, tmap, n_outer, st, false, opt);

@@ -323,7 +323,8 @@ struct KAbs {
 
 // KABS = true: the spectrum of the (unmultiplied) term is multiplied by ghat(p) VV(|p|) instead of ghat(p)
 // (homogeneous absorbing-dispersive medium, Eq. 24); kappa^2 = 1 + e alpha comes from the same tables.
-template <int N, int RL, class Lay, bool TSM = false, bool KABS = false>
+// TWOF = true: lane 0 holds F[U_s u], lane 1 F[u]: lane 0 <- ghat (lane 0 + VV lane 1), lane 1 <- 0.
+template <int N, int RL, class Lay, bool TSM = false, bool KABS = false, bool TWOF = false>
 __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, const float2 *__restrict__ p2x2,
                                                float2 a_line, KAbs ka = KAbs{0.f, 0.f, 0.f, 0.f}) {
     const int base = b * RL;
@@ -379,10 +380,12 @@ __device__ __forceinline__ void pmid_conv_item(float4 *sm, int line, int b, cons
                 const float2 kn = make_float2(exp2f(0.5f * ka.nu * lg.x), exp2f(0.5f * ka.nu * lg.y));
                 const float2 k1 = make_float2(exp2f(0.5f * lg.x), exp2f(0.5f * lg.y));
                 const float2 ok = make_float2(al.x < 1.0e17f ? 1.f : 0.f, al.y < 1.0e17f ? 1.f : 0.f);
-                const float2 vr = __fmul2_rn(__fmul2_rn(__fmul2_rn(kn, k1), f2(ka.B)), ok);                    // Re VV/k0^2
-                const float2 vi = __fmul2_rn(neg2(__ffma2_rn(kn, f2(ka.A), f2(ka.e))), ok);                    // Im VV/k0^2
+                float2 vr = __fmul2_rn(__fmul2_rn(__fmul2_rn(kn, k1), f2(ka.B)), ok);                    // Re VV/k0^2
+                float2 vi = __fmul2_rn(neg2(__ffma2_rn(kn, f2(ka.A), f2(ka.e))), ok);                    // Im VV/k0^2
+                if (TWOF) { vr.x = 1.f; vi.x = 0.f; }   // lane 0 carries the spatial term: no multiplier
                 w = P2{__ffma2_rn(w.re, vr, neg2(__fmul2_rn(w.im, vi))), __ffma2_rn(w.re, vi, __fmul2_rn(w.im, vr))};
             }
+            if (TWOF) w = P2{make_float2(w.re.x + w.re.y, 0.f), make_float2(w.im.x + w.im.y, 0.f)};
             u[k] = w;
         }
         pbfly<RL, +1>(u);

@@ -56,7 +56,7 @@ struct ColArgs {
     float inv_e;            // k0^2/eps = 1/damping
     KAbs kabs;              // k-space multiplier potential of Eq. 24 (k_conv<..., KABS = true> only)
     int masked;             // periodic boundary: axis tables mask the odd padded frequencies (general k_conv)
-    int per;                // periodic boundary, unpadded form (k_conv<..., PER = true>; 2-D)
+    int per;                // 1: periodic boundary, unpadded form (k_conv<..., PER>; 2-D); 2: its two-field form (TWOF)
     Luts lut;
     const Ctl *ctl;
 };
@@ -191,7 +191,7 @@ struct RowArgs {
     float2 *ucbs;         // CBS scheme: [rows][N] current term u_n (read and replaced); nullptr for TBS
     float inv_e;          // CBS: k0^2/eps
     int do_fwd;           // 0: stop after the inverse half (tbs_apply_green)
-    int per;              // periodic boundary, unpadded form (k_row<..., PER = true>): W is [rows][N]
+    int per;              // 1: periodic boundary, unpadded form (k_row<..., PER>): W is [rows][N]; 2: two-field form (TWOF)
     double *norms;        // [max_terms+1][2] sum |u|^2, sum |p|^2
     double *history;      // [max_terms+1]
     Ctl *ctl;
@@ -222,8 +222,13 @@ struct RowArgs {
 // PER = true: the periodic (unpadded) form (Eq. 19, Alg. 1 l.36-38): one length-N transform per grid
 // row, W is [rows][N], and the two lanes of every packed value are two adjacent grid rows (a line slot = rows
 // 2s, 2s + 1); first/last-stage table with w_N^(k t) in both lanes, no padding twist, no crop.
-template <int N, int GROUPS, int MINB, bool FIRST, bool GEN, bool PER = false>
+// TWOF = true (periodic boundary with the k-space multiplier potential AND a spatial scatterer term): the two lanes
+// are two FIELDS of the same grid row, U_s u_n and u_n, transformed together so that k_conv can form
+// ghat (F[U_s u_n] + VV F[u_n]) (Eq. 24 plus the U_s term of Eq. 25); W keeps the padded layout (column 2q + h =
+// field h at x-frequency q); only lane 0 comes back from the inverse transform.
+template <int N, int GROUPS, int MINB, bool FIRST, bool GEN, bool PER = false, bool TWOF = false>
 __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) : 32), MINB) k_row(RowArgs a) {
+    static_assert(!(PER && TWOF), "one meaning of the lanes at a time");
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
@@ -367,12 +372,14 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
             // x[h][j]: line h of the slot (the one padded line, or the two grid rows of the periodic form) at
             // position t + j*S1 -- first the inverse transform's output, then the input of the forward half
             float2 x[NR][R1];
+            float2 xf[R1];  // TWOF: lane 1 -- the inverse transform's unused lane, then the field u itself
             float2 wre[R1], wim[R1];
             load_tw_ab<R1, S1>(wre, wim, a.lut.AB, t);
             constexpr int pi = EARLY ? 1 : 0;
             const int ii = it * pi;  // slot of this item's p and V values
             if (!FIRST) {
                 if (PER) plast_inv_2l<N, R1, Lay>(x[0], x[NR - 1], l, t, wk, wre, wim);
+                else if (TWOF) plast_inv_2l<N, R1, Lay>(x[0], xf, l, t, wk, wre, wim);
                 else plast_inv_tw<N, R1, Lay>(x[0], l, t, wk, wre, wim);
             }
 #pragma unroll
@@ -383,6 +390,7 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
                     for (int j = 0; j < R1; ++j) {
                         const float2 v = ld_stream_nc(&a.src[(long long)grow * N + t + j * S1]);
                         x[h][j] = make_float2(v.x * a.src_scale, v.y * a.src_scale);
+                        if (TWOF) xf[j] = make_float2(0.f, 0.f);  // term 0 is u_0 = A G S: nothing for the multiplier
                     }
                     continue;
                 }
@@ -438,10 +446,14 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
                     }
                 }
 #pragma unroll
-                for (int j = 0; j < R1; ++j) x[h][j] = cmul(vpot[ii][j], uv[j]);
+                for (int j = 0; j < R1; ++j) {
+                    x[h][j] = cmul(vpot[ii][j], uv[j]);
+                    if (TWOF) xf[j] = uv[j];
+                }
             }
             if (!FIRST && !a.do_fwd) continue;
             if (PER) pfirst_fwd_2l<N, R1, Lay>(x[0], x[NR - 1], l, t, wk, wre, wim);
+            else if (TWOF) pfirst_fwd_2l<N, R1, Lay>(x[0], xf, l, t, wk, wre, wim);
             else pfirst_fwd_tw<N, R1, Lay>(x[0], l, t, wk, wre, wim);
         }
         group_sync<GT>(g);
@@ -548,8 +560,11 @@ __global__ void __launch_bounds__(GROUPS * (row_tpl_of(N) >= 32 ? row_tpl_of(N) 
 // length-N transform per column, and the two lanes of every packed value are the two columns of a 16-byte chunk
 // of the tile -- T/2 line slots per tile, the tile buffer read and written 16 bytes at a time, half the columns
 // and half the arithmetic per column of the padded form.  2-D only (a.p2_outer is not read).
-template <int N, int T, int MINB, bool KABS, bool PER = false>
+// TWOF = true (with PER): the two columns of a chunk are the two fields of k_row<..., TWOF> at one x-frequency; the
+// fused stage multiplies lane 1 by VV as well, adds it to lane 0 and clears it.
+template <int N, int T, int MINB, bool KABS, bool PER = false, bool TWOF = false>
 __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(ColArgs a, const __grid_constant__ CUtensorMap tmap) {
+    static_assert(!TWOF || (PER && KABS), "the two-field form runs on the periodic kernels with the multiplier");
     using P = Radix<N>;
     constexpr int R1 = P::R1, R2 = P::R2, RL = P::RL;
     constexpr int R2s = R2 > 0 ? R2 : 2;
@@ -690,12 +705,12 @@ __global__ void __launch_bounds__((PER ? T / 2 : T) * tpl_of(N), MINB) k_conv(Co
             if (!KABS) a_line = line_alpha(inner0, outer);
             float2 a_line2 = f2(a_line);
             // periodic form: the slot's two columns; the x table holds the N-grid value at entries 2q and 2q + 1
-            if (PER) a_line2 = make_float2((__ldg(&a.p2_inner[2 * (inner0 + 2 * line)]) - 1.0f) * a.inv_e,
-                                           (__ldg(&a.p2_inner[2 * (inner0 + 2 * line + 1)]) - 1.0f) * a.inv_e);
+            if (PER) a_line2 = make_float2((__ldg(&a.p2_inner[(TWOF ? 1 : 2) * (inner0 + 2 * line)]) - 1.0f) * a.inv_e,
+                                           (__ldg(&a.p2_inner[(TWOF ? 1 : 2) * (inner0 + 2 * line + 1)]) - 1.0f) * a.inv_e);
             KAbs ka = a.kabs;
             if (KABS && a.ctl->term == 0) ka.nu = 0.f;  // term 0 is u_0 = A G S: the plain Green's spectrum
 #pragma unroll 1
-            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS>(wk, line, b, p2_tab, a_line2, ka);
+            for (int b = lt; b < N / RL; b += TPL) pmid_conv_item<N, RL, Lay, P2SM, KABS, TWOF>(wk, line, b, p2_tab, a_line2, ka);
         }
         if (WL) __syncwarp();
         else group_sync<GT>(g);

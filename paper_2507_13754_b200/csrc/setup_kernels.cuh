@@ -123,6 +123,15 @@ __global__ void k_potential(float2 *V, const float *c, const float *alpha0_map, 
     V[i] = make_float2((float)((kr * kr - ki * ki - k2) / k2), (float)((2.0 * kr * ki) / k2 - damping));
 }
 
+// Spatial part of the potential next to the k-space multiplier of Eq. 24: U_s/k0^2 = ((w/c)^2 - k0^2)/k0^2, real
+// (Eq. 25 without the -i eps, which the multiplier carries).
+__global__ void k_scatterer_potential(float2 *V, const float *c, double omega, double k0, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double kr = omega / (double)c[i];
+    V[i] = make_float2((float)((kr * kr - k0 * k0) / (k0 * k0)), 0.f);
+}
+
 // Raw V (1/m^2) -> V/k0^2
 __global__ void k_scale_complex(float2 *dst, const float2 *src, double s, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -82,6 +82,7 @@ struct tbs_plan {
     size_t small_bytes = 0;      // device bytes outside the workspace (tables, control)
     int graph_batch = 16;
     int concurrency = kMaxSlots;
+    int twof = 0;                // tbs_set_kspace_scatterer: the two-field form of the periodic kernels
     int overlap = 0;             // programmatic dependent launch of the term kernels (measured slower: off)
     int scheme = TBS_SCHEME_BORN;
     int boundary = TBS_BOUNDARY_PAD;
@@ -128,6 +129,9 @@ inline size_t align_up(size_t v) { return (v + kWsAlign - 1) / kWsAlign * kWsAli
 // Periodic boundary in 2-D: the unpadded kernels (one N-point transform per line, W1 is [ny][nx]); in 3-D the
 // padded kernels with masked axis tables.
 bool per_mode(const tbs_plan *pl) { return pl->boundary == TBS_BOUNDARY_PERIODIC && pl->ndim == 2; }
+// How the kernels use the two lanes of a packed value: 0 the parity halves of a padded line, 1 two lines of the
+// unpadded periodic form, 2 two fields of one line (k-space multiplier plus a scatterer, periodic form).
+int lane_mode(const tbs_plan *pl) { return per_mode(pl) ? (pl->twof ? 2 : 1) : 0; }
 
 size_t w1_elems(const tbs_plan *pl) { return (size_t)pl->n[1] * pl->n[2] * 2 * pl->n[0]; }
 size_t w2_elems(const tbs_plan *pl) { return pl->ndim == 3 ? (size_t)pl->n[2] * 2 * pl->n[1] * 2 * pl->n[0] : 0; }
@@ -166,7 +170,7 @@ void destroy_graphs(tbs_plan *pl) {
 // form) in 2-D, W2 in 3-D.
 tbs_status make_tensor_maps(tbs_plan *pl) {
     if (!pl->ws) return TBS_OK;
-    const long long mx = (per_mode(pl) ? 1LL : 2LL) * pl->n[0], my = 2LL * pl->n[1];
+    const long long mx = (lane_mode(pl) == 1 ? 1LL : 2LL) * pl->n[0], my = 2LL * pl->n[1];
     for (int i = 0; i < pl->nslots; ++i) {
         Slot &s = pl->slot[i];
         if (pl->ndim == 2) CU(pl, make_conv_tensor_map(&s.conv_map, s.W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
@@ -213,7 +217,7 @@ void fill_row_args(tbs_plan *pl, Freq &f, Slot &s, RowArgs &a, const float2 *src
     a.scale = (float)(1.0 / (8.0 * (double)pl->npts) * (pl->ndim == 2 ? 2.0 : 1.0) / pl->damping);
     if (pl->boundary == TBS_BOUNDARY_PERIODIC) a.scale *= (float)(1 << pl->ndim);  // the odd half carries nothing
     a.do_fwd = do_fwd;
-    a.per = per_mode(pl);
+    a.per = lane_mode(pl);
     a.norms = s.norms;
     a.history = s.history;
     a.ctl = f.ctl;
@@ -223,13 +227,13 @@ void fill_row_args(tbs_plan *pl, Freq &f, Slot &s, RowArgs &a, const float2 *src
 // Column / plane passes of one term (K2 in 2-D; y-forward, z-conv, y-inverse in 3-D).
 cudaError_t launch_mid_passes(tbs_plan *pl, Freq &f, Slot &s, cudaStream_t st, int which = -1, LaunchOpt opt = LaunchOpt()) {
     const int nx = pl->n[0], ny = pl->n[1], nz = pl->n[2];
-    const long long mx = (per_mode(pl) ? 1LL : 2LL) * nx, my = 2LL * ny;
+    const long long mx = (lane_mode(pl) == 1 ? 1LL : 2LL) * nx, my = 2LL * ny;
     ColArgs a;
     memset(&a, 0, sizeof a);
     a.ctl = f.ctl;
     a.inv_e = (float)(1.0 / pl->damping);
     a.kabs = f.kabs;
-    a.per = per_mode(pl);
+    a.per = lane_mode(pl);
     a.masked = pl->boundary == TBS_BOUNDARY_PERIODIC && !a.per;
     a.inner_len = (int)mx;
     cudaError_t e = cudaSuccess;
@@ -521,6 +525,12 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
         return fail(pl, TBS_ERR_INVALID_ARG, "the k-space multiplier potential is not combined with TBS_SCHEME_CBS");
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;
+    CU(pl, cudaDeviceSynchronize());
+    if (pl->twof) {
+        pl->twof = 0;   // back to the multiplier alone (or to the spatial potential): W is one field wide again
+        tbs_status ms = make_tensor_maps(pl);
+        if (ms != TBS_OK) return ms;
+    }
     for (auto &f : pl->fr) {
         if (alpha0_si == 0.0) {
             if (f.kabs.nu > 0.f) f.have_V = false;  // the spatial potential has to be set again
@@ -547,6 +557,10 @@ tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
     if (!pl || (boundary != TBS_BOUNDARY_PAD && boundary != TBS_BOUNDARY_PERIODIC)) return TBS_ERR_INVALID_ARG;
     CU(pl, cudaDeviceSynchronize());
     pl->boundary = boundary;
+    if (pl->twof && !per_mode(pl)) {   // the two-field form exists on the periodic kernels only
+        pl->twof = 0;
+        for (auto &f : pl->fr) f.have_V = false;
+    }
     for (auto &f : pl->fr) CU(pl, fill_axis_tables(pl, f));
     // first/last-stage twiddles: the odd lane carries the padding twist, or (unpadded periodic form) a second line
     for (int a = 0; a < pl->ndim; ++a) {
@@ -602,6 +616,38 @@ static void drop_kspace_potential(tbs_plan *pl, Freq &f) {
         f.kabs = KAbs{0.f, 0.f, 0.f, 0.f};
         destroy_graphs(pl);
     }
+    if (pl->twof) {
+        cudaDeviceSynchronize();
+        pl->twof = 0;
+        make_tensor_maps(pl);
+        destroy_graphs(pl);
+    }
+}
+
+tbs_status tbs_set_kspace_scatterer(tbs_plan *pl, const float *c, void *stream) {
+    if (!pl || !c) return TBS_ERR_INVALID_ARG;
+    if (!per_mode(pl))
+        return fail(pl, TBS_ERR_INVALID_ARG, "the multiplier plus a scatterer runs on the periodic boundary in 2-D (the paper's form)");
+    for (auto &f : pl->fr)
+        if (!(f.kabs.nu > 0.f)) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_kspace_absorption first");
+    if (pl->scheme == TBS_SCHEME_CBS) return fail(pl, TBS_ERR_INVALID_ARG, "not combined with TBS_SCHEME_CBS");
+    tbs_status ws = ensure_workspace(pl);
+    if (ws != TBS_OK) return ws;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(pl, cudaDeviceSynchronize());
+    for (auto &f : pl->fr) {
+        k_scatterer_potential<<<nblk(pl->npts, 256), 256, 0, st>>>(f.V, c, f.omega, f.k0, pl->npts);
+        f.have_V = true;
+    }
+    CU(pl, cudaGetLastError());
+    CU(pl, cudaStreamSynchronize(st));
+    if (!pl->twof) {
+        pl->twof = 1;
+        tbs_status ms = make_tensor_maps(pl);
+        if (ms != TBS_OK) return ms;
+    }
+    destroy_graphs(pl);
+    return TBS_OK;
 }
 
 tbs_status tbs_set_medium(tbs_plan *pl, const float *c, const float *rho, const float *alpha0_map,

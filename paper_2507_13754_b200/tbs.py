@@ -130,6 +130,10 @@ class Plan:
         """tbs_set_kspace_absorption: homogeneous power-law medium as the k-space multiplier of Eq. 24."""
         self._check(self._L.tbs_set_kspace_absorption(self._h, float(alpha0_si), float(nu), int(bool(dispersive))))
 
+    def set_kspace_scatterer(self, c):
+        """tbs_set_kspace_scatterer: a sound-speed map next to the k-space multiplier (periodic boundary, 2-D)."""
+        self._check(self._L.tbs_set_kspace_scatterer(self._h, _dev_ptr(self._map(c, "c")), _stream_ptr()))
+
     def set_boundary(self, boundary):
         """tbs_set_boundary: "pad" (zero-pad/crop, default) or "periodic" (the paper's N-grid FFTs)."""
         code = {"pad": 0, "periodic": 1}[boundary] if isinstance(boundary, str) else int(boundary)

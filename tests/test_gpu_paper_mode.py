@@ -320,3 +320,57 @@ def test_paper_absorbing_rows_of_table_3_with_the_kspace_multiplier(golden):
         hi = 1.1 * max(golden[f"iters_{key}_gpu"], golden[f"iters_{key}_cpu"])
         assert lo <= n <= hi, (key, n)
         del plan
+
+
+@pytest.mark.parametrize("N,v_s", [(128, 1650.0), (512, 1350.0)])
+def test_kspace_multiplier_plus_scatterer_matches_oracle(N, v_s):
+    """A disc scatterer (Eqs. 25-26, v_s of Table 3) inside the absorbing-dispersive medium of
+    Eq. 24: tbs_set_kspace_absorption + tbs_set_kspace_scatterer on the periodic grid against the
+    oracle's solve_kspace(..., Us=...), L2 criterion and the paper's Eq. 30 row criterion."""
+    from paper_2507_13754_b200.tbs import Plan, TbsError
+    f, c0 = 1.0e6, 1500.0
+    dx = c0 / f / 8.0
+    a0, nu, abl = 4.0e-9, 1.5, N // 8
+    rows = np.arange(N // 2 - N // 10, N // 2 + N // 10 + 1)
+    pos = np.stack([np.full(rows.size, (abl + 5) * dx), rows * dx], 1)
+    amp = np.full((1, rows.size), -1.0e6j, dtype=np.complex64)
+    yy, xx = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    disc = (xx - 0.6 * N) ** 2 + (yy - 0.45 * N) ** 2 <= (N / 16) ** 2
+    c = np.where(disc, v_s, c0).astype(np.float32)
+    k0, eps = R.wavenumber(f, c0, 0.8)
+    g = R.green_spectrum((N, N), dx, k0, eps)
+    VV = R.kspace_potential((N, N), dx, a0, nu, f, c0, 0.8)
+    Us = (2 * np.pi * f / c.astype(np.float64)) ** 2 - k0 * k0
+    S = R.deposit((N, N), dx, pos, amp[0])
+    win = tuple(R.abl_window(N, abl) for _ in range(2))
+    plan = Plan((N, N), dx, [f], c0, 0.8)
+    with pytest.raises(TbsError):
+        plan.set_kspace_scatterer(torch.from_numpy(c).cuda())      # needs the periodic boundary ...
+    plan.set_boundary("periodic")
+    with pytest.raises(TbsError):
+        plan.set_kspace_scatterer(torch.from_numpy(c).cuda())      # ... and the multiplier
+    plan.set_abl(abl, 9.666)
+    plan.set_kspace_absorption(a0, nu)
+    plan.set_source(pos, amp)
+    alone = plan.solve(3000, 1e-6)
+    plan.set_kspace_scatterer(torch.from_numpy(c).cuda())
+    res = plan.solve(3000, 1e-6)
+    ref = R.solve_kspace(S, g, VV, 3000, 1e-6, pad=1, windows=win, Us=Us)
+    assert res.status == 0 and ref.status == R.OK
+    assert abs(int(res.n_terms[0]) - ref.n_terms) <= 1, (int(res.n_terms[0]), ref.n_terms)
+    compare_fields(res.p[0].cpu().numpy(), ref.p, "Eq. 24 + scatterer")
+    compare_history(res.history[0], ref.history, min(int(res.n_terms[0]), ref.n_terms))
+    # the scatterer is really in: the field differs from the multiplier-only run by far more than the tolerance
+    assert float((res.p - alone.p).abs().max() / alone.p.abs().max()) > 1e-2
+    # Eq. 30 on the centre row (the paper's criterion)
+    plan.set_criterion("l1_row", N // 2)
+    res30 = plan.solve(2000, 1e-5)
+    ref30 = R.solve_kspace(S, g, VV, 2000, 1e-5, pad=1, windows=win, row=N // 2, Us=Us)
+    assert abs(int(res30.n_terms[0]) - ref30.n_terms) <= 1
+    compare_fields(res30.p[0].cpu().numpy(), ref30.p, "Eq. 24 + scatterer, Eq. 30")
+    # the multiplier alone again: same result as before the scatterer was set
+    plan.set_criterion("l2_grid")
+    plan.set_kspace_absorption(a0, nu)
+    again = plan.solve(3000, 1e-6)
+    assert int(again.n_terms[0]) == int(alone.n_terms[0])
+    assert float((again.p - alone.p).abs().max() / alone.p.abs().max()) < 1e-6
