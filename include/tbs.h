@@ -180,6 +180,16 @@ tbs_status tbs_solve(tbs_plan *plan, int max_terms, double tol, float *p_out, do
 tbs_status tbs_solve_host(tbs_plan *plan, int max_terms, double tol, float *p_out_host,
                           double *history, int32_t *n_terms, void *stream);
 
+/* Continue a series that stopped at its cap (the natural call after TBS_NOT_CONVERGED; the paper caps at 2000
+ * iterations): single-frequency plans only, and only directly after the tbs_solve* that returned
+ * TBS_NOT_CONVERGED -- any call that changes the medium, source, options, workspace or the running field in between
+ * gives TBS_ERR_NOT_READY.  max_terms is the new cap on the TOTAL number of terms (> the terms already summed);
+ * history [max_terms+1] receives the whole history, n_terms the total.  The partial sum, the transformed V u_n of the
+ * next term and the norms are still on the device, so the result equals one uninterrupted tbs_solve(max_terms, tol)
+ * term for term. */
+tbs_status tbs_solve_resume(tbs_plan *plan, int max_terms, double tol, float *p_out, double *history,
+                            int32_t *n_terms, void *stream);
+
 /* Nonlinear case (Eq. 27b, 229 Eq. 28b, 266): solve `p1` (fundamental, nfreq = 1),
  * optionally rescale it so that max|p1| over the row/plane `ref_row` equals surface_pressure_pa
  * (<= 0: no rescale), form S2 = -xi (2w)^2 p1^2/2 with xi = beta/(rho0 c0^4), and solve `p2`

@@ -17,7 +17,7 @@ SYMBOLS = [
     "tbs_version", "tbs_plan_create", "tbs_plan_destroy", "tbs_plan_workspace_bytes", "tbs_plan_set_workspace",
     "tbs_plan_device_bytes", "tbs_grid_harmonic_frequency", "tbs_set_concurrency", "tbs_set_launch_overlap", "tbs_last_error",
     "tbs_set_abl", "tbs_set_scheme", "tbs_set_boundary", "tbs_set_criterion", "tbs_set_kspace_absorption", "tbs_set_kspace_scatterer", "tbs_set_medium", "tbs_set_medium_host", "tbs_set_potential", "tbs_set_source",
-    "tbs_set_source_field", "tbs_solve", "tbs_solve_host", "tbs_solve_second_harmonic", "tbs_solve_harmonics",
+    "tbs_set_source_field", "tbs_solve", "tbs_solve_host", "tbs_solve_resume", "tbs_solve_second_harmonic", "tbs_solve_harmonics",
     "tbs_apply_green", "tbs_get_potential", "tbs_get_source", "tbs_green_spectrum",
     "tbs_last_launch_count", "tbs_last_loop_ms", "tbs_profile_term", "tbs_set_graph_batch",
 ]
@@ -66,6 +66,7 @@ def load() -> ctypes.CDLL:
     L.tbs_set_source_field.argtypes = [vp, i32, vp, vp]
     L.tbs_solve.argtypes = [vp, i32, dbl, vp, dp, ip, vp]
     L.tbs_solve_host.argtypes = [vp, i32, dbl, vp, dp, ip, vp]
+    L.tbs_solve_resume.argtypes = [vp, i32, dbl, vp, dp, ip, vp]
     L.tbs_solve_second_harmonic.argtypes = [vp, vp, i32, dbl, i32, dbl, vp, vp, dp, dp, ip, ip, vp]
     L.tbs_solve_harmonics.argtypes = [ctypes.POINTER(vp), i32, i32, dbl, i32, dbl, ctypes.POINTER(vp),
                                       ctypes.POINTER(dp), ip, vp]

@@ -41,7 +41,8 @@ struct Run {
     bool active = false;
 };
 
-tbs_status run_begin(tbs_plan *pl, Run &r, int ifreq, int si, cudaStream_t st, int half, int max_terms, double tol) {
+tbs_status run_begin(tbs_plan *pl, Run &r, int ifreq, int si, cudaStream_t st, int half, int max_terms, double tol,
+                     bool resume = false) {
     Freq &f = pl->fr[ifreq];
     Slot &s = pl->slot[si];
     if (!f.have_V) return fail(pl, TBS_ERR_NOT_READY, "tbs_set_medium / tbs_set_potential not called");
@@ -51,6 +52,22 @@ tbs_status run_begin(tbs_plan *pl, Run &r, int ifreq, int si, cudaStream_t st, i
     r.ifreq = ifreq; r.si = si; r.st = st; r.half = half; r.active = true;
     r.max_batches = (max_terms + 1 + batch - 1) / batch + 1;
     Ctl *h = s.h_ctl;
+    if (resume) {
+        // tbs_solve_resume: the series stopped at its cap with W1 holding the forward half of the next term, p the
+        // partial sum and norms / history the terms so far: lift the cap and go on from the term counter
+        CU(pl, cudaMemcpyAsync(&h[0], f.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+        CU(pl, cudaStreamSynchronize(st));
+        if (!h[0].done || h[0].status != TBS_NOT_CONVERGED) return fail(pl, TBS_ERR_NOT_READY, "no capped series to resume");
+        if (max_terms <= h[0].n_terms) return fail(pl, TBS_ERR_INVALID_ARG, "max_terms must exceed the %d terms already summed", h[0].n_terms);
+        r.max_batches = (max_terms - h[0].n_terms + batch - 1) / batch + 1;
+        h[0].done = 0;
+        h[0].max_terms = max_terms;
+        h[0].tol = tol;
+        h[0].status = 1;
+        CU(pl, cudaMemcpyAsync(f.ctl, &h[0], sizeof(Ctl), cudaMemcpyHostToDevice, st));
+        CU(pl, cudaEventRecord(s.ev_t0, st));
+        return TBS_OK;
+    }
     memset(&h[0], 0, sizeof(Ctl));
     h[0].max_terms = max_terms;
     h[0].tol = tol;
@@ -135,14 +152,17 @@ tbs_status worst(tbs_status a, tbs_status b) {
 // SMs, so that the HBM-bound passes of one member overlap the FP32-bound convolution pass of another; a member that
 // has converged hands its slot to the next frequency, the last one alone goes back to full-width grids.
 tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool out_is_host,
-                     double *history, int32_t *n_terms, cudaStream_t st) {
+                     double *history, int32_t *n_terms, cudaStream_t st, bool resume = false) {
     if (!pl || max_terms < 0 || !(tol >= 0) || !p_out || !history || !n_terms) return TBS_ERR_INVALID_ARG;
+    if (resume && (pl->fr.size() != 1 || pl->resume_epoch != pl->epoch))
+        return fail(pl, TBS_ERR_NOT_READY, "tbs_solve_resume: the last call was not a capped solve of this single-frequency plan");
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;
     pl->launches = 0;
     pl->loop_ms = 0;
-    tbs_status hs = ensure_history(pl, max_terms);
+    tbs_status hs = ensure_history(pl, max_terms, resume);
     if (hs != TBS_OK) return hs;
+    pl->resume_epoch = ~0ull;
     const int nf = (int)pl->fr.size();
     const int conc = nf > 1 ? (pl->concurrency < pl->nslots ? pl->concurrency : pl->nslots) : 1;
     tbs_status res = TBS_OK;
@@ -157,7 +177,7 @@ tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool
     auto start_next = [&](int si) -> tbs_status {
         if (next >= nf) return TBS_OK;
         const int half = forked && (live + 1 > 1 || nf - next > 1) ? 1 : 0;
-        tbs_status s = run_begin(pl, run[si], next, si, forked ? pl->slot[si].own_stream : st, half, max_terms, tol);
+        tbs_status s = run_begin(pl, run[si], next, si, forked ? pl->slot[si].own_stream : st, half, max_terms, tol, resume);
         if (s == TBS_OK) { ++next; ++live; }
         return s;
     };
@@ -211,6 +231,7 @@ tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool
         cudaEventElapsedTime(&ms, pl->ev_b0, pl->ev_b1);
         pl->loop_ms = ms;   // members overlap: device time of the whole batch
     }
+    if (nf == 1 && res == TBS_NOT_CONVERGED) pl->resume_epoch = pl->epoch;   // tbs_solve_resume may go on from here
     return res;
 }
 
@@ -228,7 +249,13 @@ tbs_status tbs_solve_host(tbs_plan *pl, int max_terms, double tol, float *p_out_
     return solve_all(pl, max_terms, tol, p_out_host, true, history, n_terms, (cudaStream_t)stream);
 }
 
+tbs_status tbs_solve_resume(tbs_plan *pl, int max_terms, double tol, float *p_out, double *history,
+                            int32_t *n_terms, void *stream) {
+    return solve_all(pl, max_terms, tol, p_out, false, history, n_terms, (cudaStream_t)stream, true);
+}
+
 tbs_status tbs_apply_green(tbs_plan *pl, int ifreq, const float *x, float *out, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !x || !out || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;
@@ -293,6 +320,7 @@ tbs_status tbs_solve_harmonics(tbs_plan *const *plans, int n_harm, int max_terms
         CU(p1, cudaMemcpyAsync(&bits, p1->maxbits, sizeof bits, cudaMemcpyDeviceToHost, st));
         CU(p1, cudaStreamSynchronize(st));
         if (bits == 0u) return fail(p1, TBS_ERR_INVALID_ARG, "the fundamental vanishes on the reference row: nothing to rescale");
+        ++p1->epoch;   // the running field no longer is the series' partial sum
         k_rescale_field<<<nblk(n, 256), 256, 0, st>>>(p1->fr[0].p, p1->maxbits, surface_pressure_pa, n);
         CU(p1, cudaGetLastError());
         CU(p1, cudaMemcpyAsync(p_out[0], p1->fr[0].p, sizeof(float2) * n, cudaMemcpyDeviceToDevice, st));
@@ -344,6 +372,7 @@ tbs_status tbs_solve_second_harmonic(tbs_plan *p1, tbs_plan *p2, int max_terms, 
 // terms has put real data in place; the stop logic is held off (Ctl::hold), since a pass repeated on its own
 // output may overflow -- which does not change what a launch costs.
 tbs_status tbs_profile_term(tbs_plan *pl, int ifreq, int reps, double out_ms[4], void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !out_ms || reps < 1 || reps > 256 || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;

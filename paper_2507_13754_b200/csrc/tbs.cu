@@ -82,6 +82,8 @@ struct tbs_plan {
     size_t small_bytes = 0;      // device bytes outside the workspace (tables, control)
     int graph_batch = 16;
     int concurrency = kMaxSlots;
+    unsigned long long epoch = 0;         // bumped by every call that changes what a series computes or its state
+    unsigned long long resume_epoch = ~0ull;  // epoch at the end of a capped single-frequency solve (tbs_solve_resume)
     int twof = 0;                // tbs_set_kspace_scatterer: the two-field form of the periodic kernels
     int overlap = 0;             // programmatic dependent launch of the term kernels (measured slower: off)
     int scheme = TBS_SCHEME_BORN;
@@ -311,20 +313,26 @@ cudaError_t set_kernel_attrs(tbs_plan *pl) {
 
 // Norm and history buffers of every slot for series of up to max_terms terms.  The captured graphs hold these
 // pointers, so a reallocation drops the graphs.
-tbs_status ensure_history(tbs_plan *pl, int max_terms) {
+tbs_status ensure_history(tbs_plan *pl, int max_terms, bool keep = false) {
     if (max_terms + 1 <= pl->hist_cap) return TBS_OK;
     destroy_graphs(pl);
-    const int cap = max_terms + 1;
+    const int cap = max_terms + 1, old_cap = pl->hist_cap;
     for (int i = 0; i < pl->nslots; ++i) {
         Slot &s = pl->slot[i];
+        double *norms = nullptr, *history = nullptr, *h_hist = nullptr;
+        CU(pl, cudaMalloc((void **)&norms, sizeof(double) * 2 * cap));
+        CU(pl, cudaMalloc((void **)&history, sizeof(double) * cap));
+        CU(pl, cudaMallocHost((void **)&h_hist, sizeof(double) * cap));
+        CU(pl, cudaMemset(norms, 0, sizeof(double) * 2 * cap));
+        CU(pl, cudaMemset(history, 0, sizeof(double) * cap));
+        if (keep && s.norms && old_cap > 0) {   // tbs_solve_resume: the series so far stays
+            CU(pl, cudaMemcpy(norms, s.norms, sizeof(double) * 2 * old_cap, cudaMemcpyDeviceToDevice));
+            CU(pl, cudaMemcpy(history, s.history, sizeof(double) * old_cap, cudaMemcpyDeviceToDevice));
+        }
         if (s.norms) cudaFree(s.norms);
         if (s.history) cudaFree(s.history);
         if (s.h_hist) cudaFreeHost(s.h_hist);
-        s.norms = nullptr; s.history = nullptr; s.h_hist = nullptr;
-        pl->hist_cap = 0;
-        CU(pl, cudaMalloc((void **)&s.norms, sizeof(double) * 2 * cap));
-        CU(pl, cudaMalloc((void **)&s.history, sizeof(double) * cap));
-        CU(pl, cudaMallocHost((void **)&s.h_hist, sizeof(double) * cap));
+        s.norms = norms; s.history = history; s.h_hist = h_hist;
     }
     pl->hist_cap = cap;
     return TBS_OK;
@@ -355,6 +363,7 @@ size_t tbs_plan_workspace_bytes(const tbs_plan *plan) {
 }
 
 tbs_status tbs_plan_set_workspace(tbs_plan *pl, void *dev_ptr, size_t bytes) {
+    if (pl) ++pl->epoch;
     if (!pl || !dev_ptr) return TBS_ERR_INVALID_ARG;
     if (((uintptr_t)dev_ptr % kWsAlign) != 0) return fail(pl, TBS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
     const size_t need = workspace_layout(pl, nullptr, false);
@@ -518,6 +527,7 @@ __global__ void k_fill_complex(float2 *dst, float2 v, long long n) {
 }
 
 tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, int dispersive) {
+    if (pl) ++pl->epoch;
     if (!pl || !(alpha0_si >= 0.0)) return TBS_ERR_INVALID_ARG;
     if (alpha0_si > 0.0 && (!(nu > 0.0) || nu > 2.0 || fabs(nu - 1.0) < 1e-9))
         return fail(pl, TBS_ERR_INVALID_ARG, "power-law exponent must lie in (0, 2] and differ from 1 (PAPER.md:53)");
@@ -554,6 +564,7 @@ tbs_status tbs_set_kspace_absorption(tbs_plan *pl, double alpha0_si, double nu, 
 }
 
 tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
+    if (pl) ++pl->epoch;
     if (!pl || (boundary != TBS_BOUNDARY_PAD && boundary != TBS_BOUNDARY_PERIODIC)) return TBS_ERR_INVALID_ARG;
     CU(pl, cudaDeviceSynchronize());
     pl->boundary = boundary;
@@ -577,6 +588,7 @@ tbs_status tbs_set_boundary(tbs_plan *pl, int boundary) {
 }
 
 tbs_status tbs_set_criterion(tbs_plan *pl, int criterion, int row) {
+    if (pl) ++pl->epoch;
     if (!pl || (criterion != TBS_CRIT_L2_GRID && criterion != TBS_CRIT_L1_ROW)) return TBS_ERR_INVALID_ARG;
     const int rows = pl->n[1] * (pl->ndim == 3 ? pl->n[2] : 1);
     if (criterion == TBS_CRIT_L1_ROW && (row < 0 || row >= rows)) return fail(pl, TBS_ERR_INVALID_ARG, "row outside the grid");
@@ -586,6 +598,7 @@ tbs_status tbs_set_criterion(tbs_plan *pl, int criterion, int row) {
 }
 
 tbs_status tbs_set_scheme(tbs_plan *pl, int scheme) {
+    if (pl) ++pl->epoch;
     if (!pl || (scheme != TBS_SCHEME_BORN && scheme != TBS_SCHEME_CBS)) return TBS_ERR_INVALID_ARG;
     if (scheme == TBS_SCHEME_CBS) {
         for (auto &f : pl->fr)
@@ -600,6 +613,7 @@ tbs_status tbs_set_scheme(tbs_plan *pl, int scheme) {
 }
 
 tbs_status tbs_set_abl(tbs_plan *pl, int cells, double zeta_half_mu) {
+    if (pl) ++pl->epoch;
     if (!pl || cells < 0) return TBS_ERR_INVALID_ARG;
     for (int a = 0; a < pl->ndim; ++a)
         if (2 * cells > pl->n[a]) return fail(pl, TBS_ERR_INVALID_ARG, "ABL wider than half the grid");
@@ -625,6 +639,7 @@ static void drop_kspace_potential(tbs_plan *pl, Freq &f) {
 }
 
 tbs_status tbs_set_kspace_scatterer(tbs_plan *pl, const float *c, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !c) return TBS_ERR_INVALID_ARG;
     if (!per_mode(pl))
         return fail(pl, TBS_ERR_INVALID_ARG, "the multiplier plus a scatterer runs on the periodic boundary in 2-D (the paper's form)");
@@ -652,6 +667,7 @@ tbs_status tbs_set_kspace_scatterer(tbs_plan *pl, const float *c, void *stream) 
 
 tbs_status tbs_set_medium(tbs_plan *pl, const float *c, const float *rho, const float *alpha0_map,
                           double alpha0_db, double y, double beta, double rho0, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !c) return TBS_ERR_INVALID_ARG;
     const bool absorbing = alpha0_map != nullptr || alpha0_db != 0.0;
     if (absorbing && fabs(y - 1.0) < 1e-9) return fail(pl, TBS_ERR_INVALID_ARG, "y = 1 is excluded (PAPER.md:53)");
@@ -689,6 +705,7 @@ tbs_status tbs_set_medium_host(tbs_plan *pl, const float *c, const float *rho, c
 }
 
 tbs_status tbs_set_potential(tbs_plan *pl, int ifreq, const float *V, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !V || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;
@@ -703,6 +720,7 @@ tbs_status tbs_set_potential(tbs_plan *pl, int ifreq, const float *V, void *stre
 }
 
 tbs_status tbs_set_source(tbs_plan *pl, int n_src, const double *pos_m, const float *amp, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || n_src < 1 || !pos_m || !amp) return TBS_ERR_INVALID_ARG;
     for (int j = 0; j < n_src; ++j)
         for (int a = 0; a < pl->ndim; ++a) {
@@ -735,6 +753,7 @@ tbs_status tbs_set_source(tbs_plan *pl, int n_src, const double *pos_m, const fl
 }
 
 tbs_status tbs_set_source_field(tbs_plan *pl, int ifreq, const float *S, void *stream) {
+    if (pl) ++pl->epoch;
     if (!pl || !S || ifreq < 0 || ifreq >= (int)pl->fr.size()) return TBS_ERR_INVALID_ARG;
     tbs_status ws = ensure_workspace(pl);
     if (ws != TBS_OK) return ws;

@@ -197,6 +197,16 @@ class Plan:
         self._check(st, allow=(OK, NOT_CONVERGED, ERR_DIVERGED))
         return SolveResult(st, p, hist, nt, self.last_loop_ms(), self.last_launch_count())
 
+    def solve_resume(self, max_terms, tol, out=None) -> SolveResult:
+        """tbs_solve_resume: continue the series the last solve() left at its cap, up to max_terms terms in all."""
+        p = out if out is not None else torch.empty((self.nfreq,) + self.shape, dtype=torch.complex64, device="cuda")
+        hist, nt = self._outs(max_terms)
+        st = self._L.tbs_solve_resume(self._h, int(max_terms), float(tol), _dev_ptr(p),
+                                      hist.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                      nt.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), _stream_ptr())
+        self._check(st, allow=(OK, NOT_CONVERGED, ERR_DIVERGED))
+        return SolveResult(st, p, hist, nt, self.last_loop_ms(), self.last_launch_count())
+
     def solve_host(self, max_terms, tol, out=None) -> SolveResult:
         p = out if out is not None else np.empty((self.nfreq,) + self.shape, dtype=np.complex64)
         hist, nt = self._outs(max_terms)

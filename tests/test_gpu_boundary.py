@@ -199,3 +199,36 @@ def test_launch_overlap_and_plain_launches_give_the_same_series():
             assert res.status == 0 and int(res.n_terms[0]) == int(base.n_terms[0]), setup
             assert float((res.p - base.p).abs().max() / base.p.abs().max()) < 1e-5, setup
             assert np.allclose(res.history, base.history, rtol=1e-5), setup
+
+
+# ------------------------------------------------------------------ resume after the cap
+@pytest.mark.parametrize("maker,kw", [(W.cfg3, {"N": 256}), (W.cfg5, {"N": 32})])
+def test_resume_after_the_cap_equals_one_uninterrupted_solve(maker, kw):
+    from paper_2507_13754_b200.tbs import TbsError
+    w = maker(**kw)
+    full = gpu_plan(w).solve(w.max_terms, w.tol)
+    assert full.status == 0
+    n = int(full.n_terms[0])
+    plan = gpu_plan(w)
+    a = plan.solve(37, w.tol)                       # stops at its cap in the middle of a graph batch
+    assert a.status == 1 and int(a.n_terms[0]) == 37
+    b = plan.solve_resume(n // 2, w.tol)            # still capped; the history buffers grow
+    assert b.status == 1 and int(b.n_terms[0]) == n // 2
+    assert np.array_equal(b.history[0][:38], a.history[0][:38])
+    c = plan.solve_resume(w.max_terms, w.tol)       # to convergence
+    assert c.status == 0 and int(c.n_terms[0]) == n
+    # same kernels, same order of operations; the two plans' sources differ by the rounding of the deposition's
+    # float atomics where sub-sources share cells (3-D), and the norms by the order of the fp64 atomics across CTAs
+    assert float((c.p - full.p).abs().max() / full.p.abs().max()) < 1e-5
+    assert np.allclose(c.history, full.history, rtol=1e-5, atol=0)
+    with pytest.raises(TbsError) as e:
+        plan.solve_resume(w.max_terms, w.tol)       # nothing capped to continue
+    assert e.value.status == -3
+    d = plan.solve(20, w.tol)
+    assert d.status == 1
+    plan.set_abl(4)                                 # any change in between invalidates the state
+    with pytest.raises(TbsError):
+        plan.solve_resume(100, w.tol)
+    ref = oracle_run(w, w.max_terms, w.tol)
+    assert abs(n - ref.n_terms) <= 1
+    compare_fields(c.p[0].cpu().numpy(), ref.p, "resumed")
