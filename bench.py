@@ -48,10 +48,14 @@ NCU_COUNTS = os.path.join(ROOT, "profiles", "r02_ncu_counts.json")
 CSRC = os.path.join(ROOT, "paper_2507_13754_b200", "csrc")
 
 
+KERNEL_SOURCES = ("dispatch.cuh", "dispatch_impl.cuh", "fft_engine.cuh", "fft_engine_x2.cuh", "kernels.cuh")
+
+
 def kernel_source_sha():
-    """Identifies the kernels being timed: sha256 over the CUDA sources, in name order."""
+    """Identifies the term kernels being timed: sha256 over their sources and launch configurations (the host-side
+    files tbs.cu / solve.inl and the setup kernels do not change what k_row, k_conv and k_col execute)."""
     h = hashlib.sha256()
-    for name in sorted(os.listdir(CSRC)):
+    for name in KERNEL_SOURCES:
         with open(os.path.join(CSRC, name), "rb") as fh:
             h.update(name.encode() + b"\0" + fh.read())
     return h.hexdigest()[:16]
