@@ -76,9 +76,8 @@ size_t tbs_plan_device_bytes(const tbs_plan *plan);
 double tbs_grid_harmonic_frequency(int m, double c0, int n, double dx_m);
 
 /* Frequency batch (nfreq > 1): how many members are solved at once, 1 or 2 (default 2).  With 2, two series run
- * on streams of the plan's own with grids sized for half of the SMs each, so that the HBM-bound passes of one
- * overlap the FP32-bound convolution pass of the other; a member that has stopped hands its place to the next
- * frequency.  The paper's harmonic loop is sequential. */
+ * on streams of the plan's own, so that the HBM-bound passes of one overlap the FP32-bound convolution pass of
+ * the other as SM resources free up; a member that has stopped hands its place to the next frequency.  The paper's harmonic loop is sequential. */
 tbs_status tbs_set_concurrency(tbs_plan *plan, int members);
 
 /* Text of the last error on this plan (plan-owned storage, valid until the next call). */

@@ -148,9 +148,10 @@ tbs_status worst(tbs_status a, tbs_status b) {
 }
 
 // All frequencies of the plan.  One frequency: the series runs on the caller's stream on slot 0.  Several: up to
-// `concurrency` members are in flight at once, each on its slot's own stream with grids sized for its share of the
-// SMs, so that the HBM-bound passes of one member overlap the FP32-bound convolution pass of another; a member that
-// has converged hands its slot to the next frequency, the last one alone goes back to full-width grids.
+// `concurrency` members are in flight at once, each on its slot's own stream, so that the HBM-bound passes of one
+// member overlap the FP32-bound convolution pass of another; a member that has converged hands its slot to the
+// next frequency.
+constexpr bool kHalfWidthBatchGrids = false;
 tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool out_is_host,
                      double *history, int32_t *n_terms, cudaStream_t st, bool resume = false) {
     if (!pl || max_terms < 0 || !(tol >= 0) || !p_out || !history || !n_terms) return TBS_ERR_INVALID_ARG;
@@ -176,7 +177,10 @@ tbs_status solve_all(tbs_plan *pl, int max_terms, double tol, float *p_out, bool
     }
     auto start_next = [&](int si) -> tbs_status {
         if (next >= nf) return TBS_OK;
-        const int half = forked && (live + 1 > 1 || nf - next > 1) ? 1 : 0;
+        // Grid width of members in flight together.  Measured on B200 (two members): full-width grids (the block
+        // scheduler interleaves the two members' CTAs as SM resources free up) 9.97 -> 9.54 s on the 16-frequency
+        // 256^3 batch and 126 -> 93 ms at 64^3; grids sized for half of the SMs each 9.70 -> 9.86 s and 126 -> 93 ms.
+        const int half = kHalfWidthBatchGrids && forked && (live + 1 > 1 || nf - next > 1) ? 1 : 0;
         tbs_status s = run_begin(pl, run[si], next, si, forked ? pl->slot[si].own_stream : st, half, max_terms, tol, resume);
         if (s == TBS_OK) { ++next; ++live; }
         return s;
