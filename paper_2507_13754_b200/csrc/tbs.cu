@@ -17,7 +17,7 @@ using namespace tbs;
 namespace {
 
 constexpr double kPi = 3.14159265358979323846;
-constexpr int kMaxSlots = 2;          // members of a frequency batch in flight at once
+constexpr int kMaxSlots = 4;          // members of a frequency batch in flight at once, at most
 constexpr size_t kWsAlign = 256;      // alignment of every workspace region (TMA / bulk copies need 16)
 
 // A CUDA graph of `batch` Born terms of one frequency on one slot at one grid width.
@@ -45,6 +45,7 @@ struct Freq {
 struct Slot {
     float2 *W1 = nullptr;   // [nz*ny][2 nx]                    (workspace)
     float2 *W2 = nullptr;   // 3-D: [nz][2 ny][2 nx]            (workspace)
+    bool own_w = false;     // slots beyond the second: W1/W2 allocated by the plan (tbs_set_concurrency)
     CUtensorMap conv_map;   // tensor map of the array k_conv transforms in place (W1 in 2-D, W2 in 3-D)
     double *norms = nullptr, *history = nullptr;   // device, hist_cap entries
     double *h_hist = nullptr;                      // pinned
@@ -62,7 +63,8 @@ struct tbs_plan {
     double dx = 0, c0 = 0, damping = 0;
     double beta = 1.0, rho0 = 1000.0;
     std::vector<Freq> fr;
-    int nslots = 1;
+    int nslots = 1;              // slots with streams, events and history buffers: min(nfreq, kMaxSlots)
+    int ws_slots = 1;            // slots whose W1/W2 live in the workspace: min(nfreq, 2)
     Slot slot[kMaxSlots];
     float2 *lutA[3] = {nullptr, nullptr, nullptr};   // per axis, fft_engine.cuh "Luts"
     float2 *lutB[3] = {nullptr, nullptr, nullptr};
@@ -81,7 +83,7 @@ struct tbs_plan {
     cudaEvent_t ev_fork = nullptr, ev_b0 = nullptr, ev_b1 = nullptr;
     size_t small_bytes = 0;      // device bytes outside the workspace (tables, control)
     int graph_batch = 16;
-    int concurrency = kMaxSlots;
+    int concurrency = 2;         // members in flight (tbs_set_concurrency)
     unsigned long long epoch = 0;         // bumped by every call that changes what a series computes or its state
     unsigned long long resume_epoch = ~0ull;  // epoch at the end of a capped single-frequency solve (tbs_solve_resume)
     int twof = 0;                // tbs_set_kspace_scatterer: the two-field form of the periodic kernels
@@ -150,7 +152,7 @@ size_t workspace_layout(tbs_plan *pl, char *base, bool bind) {
         float2 *v = take((size_t)pl->npts), *s = take((size_t)pl->npts), *p = take((size_t)pl->npts);
         if (bind) { f.V = v; f.S = s; f.p = p; }
     }
-    for (int i = 0; i < pl->nslots; ++i) {
+    for (int i = 0; i < pl->ws_slots; ++i) {
         float2 *w1 = take(w1_elems(pl));
         float2 *w2 = pl->ndim == 3 ? take(w2_elems(pl)) : nullptr;
         if (bind) { pl->slot[i].W1 = w1; pl->slot[i].W2 = w2; }
@@ -175,6 +177,7 @@ tbs_status make_tensor_maps(tbs_plan *pl) {
     const long long mx = (lane_mode(pl) == 1 ? 1LL : 2LL) * pl->n[0], my = 2LL * pl->n[1];
     for (int i = 0; i < pl->nslots; ++i) {
         Slot &s = pl->slot[i];
+        if (!s.W1) continue;   // a slot beyond the second that tbs_set_concurrency has not asked for
         if (pl->ndim == 2) CU(pl, make_conv_tensor_map(&s.conv_map, s.W1, mx, pl->n[1], mx, conv_tile_width(pl->n[1])));
         else CU(pl, make_conv_tensor_map(&s.conv_map, s.W2, my * mx, pl->n[2], my * mx, conv_tile_width(pl->n[2])));
     }
@@ -404,6 +407,21 @@ tbs_status tbs_set_launch_overlap(tbs_plan *plan, int on) {
 
 tbs_status tbs_set_concurrency(tbs_plan *plan, int members) {
     if (!plan || members < 1 || members > kMaxSlots) return TBS_ERR_INVALID_ARG;
+    tbs_plan *pl = plan;
+    // the first two slots' intermediates are part of the workspace; further ones are the plan's own
+    bool grew = false;
+    for (int i = pl->ws_slots; i < members && i < pl->nslots; ++i) {
+        Slot &s = pl->slot[i];
+        if (s.W1) continue;
+        CU(pl, dmalloc(pl, &s.W1, w1_elems(pl)));
+        if (pl->ndim == 3) CU(pl, dmalloc(pl, &s.W2, w2_elems(pl)));
+        s.own_w = true;
+        grew = true;
+    }
+    if (grew) {
+        tbs_status ms = make_tensor_maps(pl);
+        if (ms != TBS_OK) return ms;
+    }
     plan->concurrency = members;
     return TBS_OK;
 }
@@ -422,6 +440,7 @@ void tbs_plan_destroy(tbs_plan *pl) {
     cudaFree(pl->maxbits);
     cudaFree(pl->stage);
     for (auto &s : pl->slot) {
+        if (s.own_w) { cudaFree(s.W1); cudaFree(s.W2); }
         cudaFree(s.norms); cudaFree(s.history);
         if (s.h_ctl) cudaFreeHost(s.h_ctl);
         if (s.h_hist) cudaFreeHost(s.h_hist);
@@ -457,7 +476,8 @@ tbs_status tbs_plan_create(tbs_plan **out, int ndim, const int32_t n[3], double 
     pl->npts = (long long)pl->n[0] * pl->n[1] * pl->n[2];
     pl->dx = dx_m; pl->c0 = c0; pl->damping = damping;
     pl->fr.resize(nfreq);
-    pl->nslots = nfreq > 1 ? kMaxSlots : 1;
+    pl->nslots = nfreq < kMaxSlots ? nfreq : kMaxSlots;
+    pl->ws_slots = nfreq < 2 ? nfreq : 2;
     tbs_status st = TBS_OK;
     auto build = [&]() -> tbs_status {
         int dev = 0;

@@ -168,6 +168,10 @@ def test_frequency_batch_solved_together_matches_per_frequency_oracle(maker, kw,
     plan = gpu_plan(w)
     res = plan.solve(w.max_terms, w.tol)          # default: two members in flight
     assert res.status == 0
+    plan.set_concurrency(4)
+    four = plan.solve(w.max_terms, w.tol)         # four in flight: slots three and four are the plan's own
+    assert np.array_equal(res.n_terms, four.n_terms)
+    assert float((res.p - four.p).abs().max() / four.p.abs().max()) < 1e-6
     plan.set_concurrency(1)
     seq = plan.solve(w.max_terms, w.tol)          # one after the other
     assert np.array_equal(res.n_terms, seq.n_terms)
